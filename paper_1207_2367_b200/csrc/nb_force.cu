@@ -1,0 +1,398 @@
+// nb_force.cu -- the evaluation step: acceleration, jerk and snap of the active particles
+// against all predicted particles.  PAPER.md:72-81 (Eq. 8-10) with the Eq. 2 softening
+// in every r_ij^2 (reading G3); split over j when the active set is
+// small (the paper's "Bfactor") followed by a fixed-order reduction of the
+// partial sums (Table 1 row 4).
+//
+// The kernel is bound by the FP64 pipe: per pair it issues
+// 32 DFMA + 11 DMUL + 10 DADD = 53 FP64 instructions (85 flops) and one MUFU.RSQ64H.
+//   - one i-particle per lane (or per group of JL lanes when m is small), its nine
+//     predicted values and nine accumulators held in registers;
+//   - the j-stream is read as packed 80-byte records staged through shared memory by 1-D
+//     bulk copies (cp.async.bulk -> UBLKCP, completion on an mbarrier), two stages deep,
+//     issued by one thread; every lane then reads the same record (LDS.128 broadcast);
+//   - 1/sqrt(s): hardware seed on the upper word (rsqrt.approx.ftz.f64 -> MUFU.RSQ64H,
+//     ~2^-21) refined by ONE third-order FP64 step y <- y + y e (1/2 + 3/8 e), e = 1 - s y^2,
+//     relative error < 2^-60 before rounding;
+//   - sums are blocked: one partial per j-tile is added to the running total, so the
+//     rounding error grows with sqrt(tile) + sqrt(#tiles) instead of sqrt(N).
+#include <stdarg.h>
+#include <stdio.h>
+
+#include "nb_internal.cuh"
+
+namespace nb {
+
+struct Acc9 {
+    double ax, ay, az, jx, jy, jz, sx, sy, sz;
+};
+
+__device__ __forceinline__ double rsqrt_seed(double s)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(s));
+    return y;
+}
+
+// One pair interaction, Eq. 8-10 in the factored form:
+//   s = |dr|^2 + eps^2, w = m_j s^(-3/2), g = -3 (dr.dv)/s, b3 = -3 beta,
+//   u = dv + g dr,  A0 = w dr,  A1 = w u,  A2 = w (da + 2 g u + b3 dr).
+// q points at the packed record {x y z vx vy vz ax ay az m} of particle j in shared memory.
+template <bool GUARD0>
+__device__ __forceinline__ void pair_body(const double xi, const double yi, const double zi,
+                                          const double vxi, const double vyi, const double vzi,
+                                          const double axi, const double ayi, const double azi,
+                                          const double *__restrict__ q, const double eps2, Acc9 &A)
+{
+    const double2 p0 = *reinterpret_cast<const double2 *>(q);
+    const double2 p1 = *reinterpret_cast<const double2 *>(q + 2);
+    const double2 p2 = *reinterpret_cast<const double2 *>(q + 4);
+    const double2 p3 = *reinterpret_cast<const double2 *>(q + 6);
+    const double2 p4 = *reinterpret_cast<const double2 *>(q + 8);
+    const double dx = p0.x - xi, dy = p0.y - yi, dz = p1.x - zi;
+    const double dvx = p1.y - vxi, dvy = p2.x - vyi, dvz = p2.y - vzi;
+    const double dax = p3.x - axi, day = p3.y - ayi, daz = p4.x - azi;
+    const double mj = p4.y;
+    const double s = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+    const double rv = fma(dx, dvx, fma(dy, dvy, dz * dvz));
+    const double vr = fma(dx, dax, fma(dy, day, fma(dz, daz, fma(dvx, dvx, fma(dvy, dvy, dvz * dvz)))));
+    double y0 = rsqrt_seed(s);
+    if (GUARD0) {  // eps = 0: a coincident pair (the self term) contributes nothing (G12)
+        if ((__double2hiint(s) | __double2loint(s)) == 0) y0 = 0.0;
+    }
+    const double y2 = y0 * y0;
+    const double e = fma(-s, y2, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    const double ye = y0 * e;
+    const double y = fma(ye, p, y0);   // s^(-1/2)
+    const double ri2 = y * y;          // 1/s
+    const double my = mj * y;
+    const double w = my * ri2;         // m_j s^(-3/2)
+    const double qq = -3.0 * ri2;
+    const double g = rv * qq;          // -3 alpha
+    const double al = g * (-1.0 / 3.0);
+    const double qv = qq * vr;
+    const double b3 = fma(al, g, qv);  // -3 beta = -3 (v^2 + r.a)/s - 3 alpha^2
+    const double g2 = g + g;
+    const double ux = fma(g, dx, dvx), uy = fma(g, dy, dvy), uz = fma(g, dz, dvz);
+    A.ax = fma(w, dx, A.ax);
+    A.ay = fma(w, dy, A.ay);
+    A.az = fma(w, dz, A.az);
+    A.jx = fma(w, ux, A.jx);
+    A.jy = fma(w, uy, A.jy);
+    A.jz = fma(w, uz, A.jz);
+    double tx = fma(g2, ux, dax), ty = fma(g2, uy, day), tz = fma(g2, uz, daz);
+    tx = fma(b3, dx, tx);
+    ty = fma(b3, dy, ty);
+    tz = fma(b3, dz, tz);
+    A.sx = fma(w, tx, A.sx);
+    A.sy = fma(w, ty, A.sy);
+    A.sz = fma(w, tz, A.sz);
+}
+
+// ---- mbarrier / bulk-copy primitives (PTX, sm_90+; SASS: SYNCS.*, UBLKCP) ---------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+            smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+
+// ---- the evaluation kernel -------------------------------------------------------------
+// grid.x: i-blocks, grid.y: j-splits.  JLT = 1: one i per thread.  JLT = 0: JL (runtime,
+// power of two <= 32) consecutive lanes share one i and stride through the tile.
+template <int NT, int TJ, int MINB, int JLT, bool GUARD0>
+__global__ void __launch_bounds__(NT, MINB)
+    k_force(const double *__restrict__ jp, const int32_t *__restrict__ active, const int m,
+            const int tiles_total, const int tiles_per_split, const int JLr, const double eps2,
+            double *__restrict__ out, const size_t cstride, const size_t sstride)
+{
+    constexpr int NS = 2;
+    constexpr uint32_t TILE_BYTES = TJ * REC * sizeof(double);
+    __shared__ __align__(128) double tile[NS][TJ * REC];
+    __shared__ __align__(8) uint64_t full[NS];
+
+    const int JL = JLT ? 1 : JLr;
+    const int tid = threadIdx.x;
+    const int slots = NT / JL;                      // i-particles per CTA
+    const int k = blockIdx.x * slots + tid / JL;    // slot in the active list
+    const int jl = tid % JL;                        // j-lane
+    const int t0 = blockIdx.y * tiles_per_split;
+    const int nt = min(tiles_per_split, tiles_total - t0);
+    const char *src = reinterpret_cast<const char *>(jp) + (size_t)t0 * TILE_BYTES;
+
+    if (tid == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) {
+        for (int st = 0; st < NS && st < nt; ++st) {
+            mbar_expect_tx(&full[st], TILE_BYTES);
+            bulk_g2s(tile[st], src + (size_t)st * TILE_BYTES, TILE_BYTES, &full[st]);
+        }
+    }
+
+    // i-particle: predicted r, v, a of active[k] (differences of PREDICTED data)
+    const int kc = min(k, m - 1);
+    const int i = active ? active[kc] : kc;
+    const double *pi = jp + (size_t)i * REC;
+    const double2 i0 = *reinterpret_cast<const double2 *>(pi);
+    const double2 i1 = *reinterpret_cast<const double2 *>(pi + 2);
+    const double2 i2 = *reinterpret_cast<const double2 *>(pi + 4);
+    const double2 i3 = *reinterpret_cast<const double2 *>(pi + 6);
+    const double i4 = pi[8];
+    const double xi = i0.x, yi = i0.y, zi = i1.x, vxi = i1.y, vyi = i2.x, vzi = i2.y;
+    const double axi = i3.x, ayi = i3.y, azi = i4;
+
+    // a warp whose slots are all beyond m only keeps the barriers company
+    const bool warp_idle = (blockIdx.x * slots + (tid & ~31) / JL) >= m;
+
+    Acc9 T = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+    for (int it = 0; it < nt; ++it) {
+        const int st = it & 1;
+        mbar_wait(&full[st], (it >> 1) & 1);
+        if (!warp_idle) {
+            Acc9 A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+            const double *q = tile[st];
+            if (JLT) {
+#pragma unroll 4
+                for (int jj = 0; jj < TJ; ++jj)
+                    pair_body<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
+            } else {
+#pragma unroll 2
+                for (int jj = jl; jj < TJ; jj += JL)
+                    pair_body<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
+            }
+            T.ax += A.ax; T.ay += A.ay; T.az += A.az;
+            T.jx += A.jx; T.jy += A.jy; T.jz += A.jz;
+            T.sx += A.sx; T.sy += A.sy; T.sz += A.sz;
+        }
+        __syncthreads();  // every warp is done reading tile[st]
+        if (tid == 0 && it + NS < nt) {
+            mbar_expect_tx(&full[st], TILE_BYTES);
+            bulk_g2s(tile[st], src + (size_t)(it + NS) * TILE_BYTES, TILE_BYTES, &full[st]);
+        }
+    }
+
+    if (!JLT) {  // fixed-order butterfly over the JL lanes that share this i
+        for (int off = JL >> 1; off > 0; off >>= 1) {
+            T.ax += __shfl_xor_sync(0xffffffffu, T.ax, off);
+            T.ay += __shfl_xor_sync(0xffffffffu, T.ay, off);
+            T.az += __shfl_xor_sync(0xffffffffu, T.az, off);
+            T.jx += __shfl_xor_sync(0xffffffffu, T.jx, off);
+            T.jy += __shfl_xor_sync(0xffffffffu, T.jy, off);
+            T.jz += __shfl_xor_sync(0xffffffffu, T.jz, off);
+            T.sx += __shfl_xor_sync(0xffffffffu, T.sx, off);
+            T.sy += __shfl_xor_sync(0xffffffffu, T.sy, off);
+            T.sz += __shfl_xor_sync(0xffffffffu, T.sz, off);
+        }
+    }
+    if (k < m && jl == 0) {
+        double *o = out + (size_t)blockIdx.y * sstride + k;
+        o[0 * cstride] = T.ax; o[1 * cstride] = T.ay; o[2 * cstride] = T.az;
+        o[3 * cstride] = T.jx; o[4 * cstride] = T.jy; o[5 * cstride] = T.jz;
+        o[6 * cstride] = T.sx; o[7 * cstride] = T.sy; o[8 * cstride] = T.sz;
+    }
+}
+
+// ---- partial-sum reduction (Table 1 row 4): f1[c][k] = sum_s part[s][c][k], s ascending ---
+// thread-per-element version: coalesced along k, used when the number of splits is small
+__global__ void k_reduce_thread(const double *__restrict__ part, const int S, const int m,
+                                const size_t cstride, const size_t sstride, double *__restrict__ f1,
+                                const size_t f1stride)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int c = blockIdx.y;
+    if (k >= m) return;
+    const double *p = part + c * cstride + k;
+    double acc = 0.0;
+    for (int s = 0; s < S; ++s) acc += p[(size_t)s * sstride];
+    f1[c * f1stride + k] = acc;
+}
+// warp-per-element version: lane l sums splits l, l+32, ... then a fixed butterfly
+__global__ void k_reduce_warp(const double *__restrict__ part, const int S, const int m,
+                              const size_t cstride, const size_t sstride, double *__restrict__ f1,
+                              const size_t f1stride)
+{
+    const int wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (wid >= 9 * m) return;
+    const int c = wid / m, k = wid - c * m;
+    const double *p = part + c * cstride + k;
+    double acc = 0.0;
+    for (int s = lane; s < S; s += 32) acc += p[(size_t)s * sstride];
+    for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+    if (lane == 0) f1[c * f1stride + k] = acc;
+}
+
+// f1[c][k] -> stage[q][k][3]  (q = 0 acc, 1 jerk, 2 snap), the caller-facing [n][3] layout
+__global__ void k_unpack_f1(const double *__restrict__ f1, const size_t f1stride, const int m,
+                            double *__restrict__ stage)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= m) return;
+#pragma unroll
+    for (int c = 0; c < 9; ++c) {
+        const int q = c / 3, d = c % 3;
+        stage[((size_t)q * m + k) * 3 + d] = f1[c * f1stride + k];
+    }
+}
+
+// ---- host side ---------------------------------------------------------------------------
+constexpr int NT_A = 128, TJ_A = 128, MINB_A = 4;   // variant A: one i per thread, m >= 128
+constexpr int NT_B = 32, TJ_B = 64, MINB_B = 16;    // variant B: one warp per CTA, small m
+
+int query_force_occupancy(nb_ctx *ctx)
+{
+    int v = 0;
+    NB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+                     &v, k_force<NT_A, TJ_A, MINB_A, 1, false>, NT_A, 0));
+    ctx->occ[0] = v > 0 ? v : 1;
+    NB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+                     &v, k_force<NT_B, TJ_B, MINB_B, 0, false>, NT_B, 0));
+    ctx->occ[1] = v > 0 ? v : 1;
+    return NB_OK;
+}
+
+// Number of j-splits.  All CTAs do the same work per tile, so the cost of a launch is
+// waves x (tiles per split + a fixed per-CTA cost `o` in tile units).  For a given number of
+// waves the best S is the largest that still fits, so only those candidates are scored.
+static int choose_split(int64_t n_iblocks, int64_t tiles, int64_t slots, int64_t s_cap)
+{
+    if (s_cap > tiles) s_cap = tiles;
+    if (s_cap > 65535) s_cap = 65535;
+    if (s_cap < 1) s_cap = 1;
+    double best = 1e300;
+    int best_s = 1;
+    for (int64_t w = 0; w <= 64; ++w) {
+        int64_t S = (w == 0) ? 1 : (w * slots) / n_iblocks;
+        if (S < 1) continue;
+        if (S > s_cap) S = s_cap;
+        const int64_t tps = (tiles + S - 1) / S;
+        S = (tiles + tps - 1) / tps;  // splits that actually get tiles
+        const int64_t waves = (n_iblocks * S + slots - 1) / slots;
+        const double cost = (double)waves * ((double)tps + 0.75) + 0.002 * (double)S;
+        if (cost < best - 1e-12) { best = cost; best_s = (int)S; }
+    }
+    return best_s;
+}
+
+template <int NT, int TJ, int MINB, int JLT>
+static void launch_variant(nb_ctx *ctx, dim3 grid, const int32_t *active, int m, int tiles_total,
+                           int tps, int JL, double *out, size_t cstride, size_t sstride)
+{
+    if (ctx->eps == 0.0)
+        k_force<NT, TJ, MINB, JLT, true><<<grid, NT, 0, ctx->stream>>>(
+            ctx->jp, active, m, tiles_total, tps, JL, ctx->eps2, out, cstride, sstride);
+    else
+        k_force<NT, TJ, MINB, JLT, false><<<grid, NT, 0, ctx->stream>>>(
+            ctx->jp, active, m, tiles_total, tps, JL, ctx->eps2, out, cstride, sstride);
+}
+
+int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m)
+{
+    if (m <= 0) return NB_OK;
+    const bool varA = (m >= 128) && !(ctx->force_jlanes > 1);
+    int JL = 1;
+    if (!varA) {
+        if (ctx->force_jlanes >= 1) JL = ctx->force_jlanes;
+        else { while (JL < 8 && m * (JL * 2) <= 32) JL *= 2; }
+    }
+    const int NT = varA ? NT_A : NT_B, TJ = varA ? TJ_A : TJ_B;
+    const int64_t slots_per_cta = NT / JL;
+    const int64_t n_ib = (m + slots_per_cta - 1) / slots_per_cta;
+    const int64_t tiles = ctx->Npad / TJ;
+    const int64_t cta_slots = (int64_t)ctx->n_sm * ctx->occ[varA ? 0 : 1];
+    const int64_t mpad = (m + 31) & ~(int64_t)31;
+    int64_t s_cap = (int64_t)((size_t)1 << 28) / (9 * mpad);  // partials <= 2 GiB
+    int S = ctx->force_split >= 1 ? (int)(ctx->force_split < tiles ? ctx->force_split : tiles)
+                                  : choose_split(n_ib, tiles, cta_slots, s_cap);
+    int64_t tps = (tiles + S - 1) / S;
+    S = (int)((tiles + tps - 1) / tps);
+
+    double *out = ctx->f1;
+    size_t cstride = (size_t)ctx->Npad, sstride = 0;
+    if (S > 1) {
+        const size_t need = (size_t)S * 9 * (size_t)mpad;
+        if (need > ctx->partials_cap) {
+            if (ctx->partials) { NB_CUDA(ctx, cudaStreamSynchronize(ctx->stream)); cudaFree(ctx->partials); }
+            ctx->partials = nullptr; ctx->partials_cap = 0;
+            size_t cap = need + need / 2;
+            NB_CUDA(ctx, cudaMalloc(&ctx->partials, cap * sizeof(double)));
+            ctx->partials_cap = cap;
+        }
+        out = ctx->partials; cstride = (size_t)mpad; sstride = 9 * (size_t)mpad;
+    }
+    dim3 grid((unsigned)n_ib, (unsigned)S, 1);
+    if (varA)
+        launch_variant<NT_A, TJ_A, MINB_A, 1>(ctx, grid, active, (int)m, (int)tiles, (int)tps, 1, out, cstride, sstride);
+    else
+        launch_variant<NT_B, TJ_B, MINB_B, 0>(ctx, grid, active, (int)m, (int)tiles, (int)tps, JL, out, cstride, sstride);
+    NB_LAUNCH_CHECK(ctx, "k_force");
+    if (S > 1) {
+        if (S < 32) {
+            dim3 g((unsigned)((m + 127) / 128), 9, 1);
+            k_reduce_thread<<<g, 128, 0, ctx->stream>>>(out, S, (int)m, cstride, sstride, ctx->f1, (size_t)ctx->Npad);
+        } else {
+            const int64_t warps = 9 * m;
+            k_reduce_warp<<<(unsigned)((warps + 7) / 8), 256, 0, ctx->stream>>>(out, S, (int)m, cstride, sstride, ctx->f1, (size_t)ctx->Npad);
+        }
+        NB_LAUNCH_CHECK(ctx, "k_reduce");
+    }
+    ctx->last_launch[0] = NT; ctx->last_launch[1] = JL; ctx->last_launch[2] = S;
+    ctx->last_launch[3] = n_ib * S; ctx->last_launch[4] = TJ;
+    ctx->n_pairs += (double)m * (double)ctx->N;
+    return NB_OK;
+}
+
+int launch_unpack_f1(nb_ctx *ctx, int64_t m)
+{
+    if (m <= 0) return NB_OK;
+    k_unpack_f1<<<(unsigned)((m + 255) / 256), 256, 0, ctx->stream>>>(ctx->f1, (size_t)ctx->Npad, (int)m, ctx->stage);
+    NB_LAUNCH_CHECK(ctx, "k_unpack_f1");
+    return NB_OK;
+}
+
+int set_err(nb_ctx *ctx, int code, const char *fmt, ...)
+{
+    if (ctx) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+}  // namespace nb

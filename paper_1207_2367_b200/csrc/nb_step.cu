@@ -1,0 +1,506 @@
+// nb_step.cu -- the O(N) and O(m) kernels around the evaluation step:
+//   predictor            Eq. 3-7      k_predict
+//   next block / gather  Table 1 row 1    k_tmin, k_count_scan, k_scatter
+//   corrector            Eq. 11-14      k_correct
+//   new time step        Eq. 15-16     new_dt() inside k_correct
+//   start-up             DESIGN.md reading G8            k_startup_commit
+// All of them stream the SoA state once; they are HBM- or latency-bound.
+#include "nb_internal.cuh"
+
+namespace nb {
+
+// ---------------------------------------------------------------------------------------
+// load: caller layout [N][3] -> SoA planes, predicted records {r, v, 0, m}; t = dt = 0
+__global__ void k_load_state(const int64_t N, const int64_t Npad, const double *__restrict__ pos,
+                             const double *__restrict__ vel, const double *__restrict__ mass_in,
+                             double *__restrict__ r, double *__restrict__ v, double *__restrict__ mass,
+                             double *__restrict__ jp)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
+    const double vx = vel[3 * i], vy = vel[3 * i + 1], vz = vel[3 * i + 2];
+    const double m = mass_in[i];
+    r[i] = x; r[Npad + i] = y; r[2 * Npad + i] = z;
+    v[i] = vx; v[Npad + i] = vy; v[2 * Npad + i] = vz;
+    mass[i] = m;
+    double2 *rec = reinterpret_cast<double2 *>(jp + i * REC);
+    rec[0] = make_double2(x, y);
+    rec[1] = make_double2(z, vx);
+    rec[2] = make_double2(vy, vz);
+    rec[3] = make_double2(0.0, 0.0);
+    rec[4] = make_double2(0.0, m);
+}
+
+int launch_load_state(nb_ctx *ctx, const double *pos, const double *vel, const double *mass_in)
+{
+    const int64_t N = ctx->N;
+    k_load_state<<<(unsigned)((N + 255) / 256), 256, 0, ctx->stream>>>(N, ctx->Npad, pos, vel, mass_in, ctx->r,
+                                                                       ctx->v, ctx->mass, ctx->jp);
+    NB_LAUNCH_CHECK(ctx, "k_load_state");
+    return NB_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// Predictor, Eq. 3-7 with the garbled dots read as the Taylor series (G1) and
+// the interval h = t - t_i for every particle (G2), in Horner form:
+//   r_p = r + h (v + h/2 (a + h/3 (j + h/4 (s + h/5 c))))
+//   v_p = v + h (a + h/2 (j + h/3 (s + h/4 c)))
+//   a_p = a + h (j + h/2 (s + h/3 c))
+// Reads 19 + 1 doubles, writes one 80-byte record: 240 B per particle.
+__global__ void k_predict(const int64_t N, const int64_t Npad, const double t,
+                          const double *__restrict__ ti, const double *__restrict__ mass,
+                          const double *__restrict__ r, const double *__restrict__ v,
+                          const double *__restrict__ a, const double *__restrict__ j,
+                          const double *__restrict__ s, const double *__restrict__ c,
+                          double *__restrict__ jp)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double h = t - ti[i];
+    const double h2 = h * 0.5, h3 = h * (1.0 / 3.0), h4 = h * 0.25, h5 = h * 0.2;
+    double rp[3], vp[3], ap[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const int64_t q = d * Npad + i;
+        const double r0 = r[q], v0 = v[q], a0 = a[q], j0 = j[q], s0 = s[q], c0 = c[q];
+        rp[d] = fma(h, fma(h2, fma(h3, fma(h4, fma(h5, c0, s0), j0), a0), v0), r0);
+        vp[d] = fma(h, fma(h2, fma(h3, fma(h4, c0, s0), j0), a0), v0);
+        ap[d] = fma(h, fma(h2, fma(h3, c0, s0), j0), a0);
+    }
+    double2 *rec = reinterpret_cast<double2 *>(jp + i * REC);
+    rec[0] = make_double2(rp[0], rp[1]);
+    rec[1] = make_double2(rp[2], vp[0]);
+    rec[2] = make_double2(vp[1], vp[2]);
+    rec[3] = make_double2(ap[0], ap[1]);
+    rec[4] = make_double2(ap[2], mass[i]);
+}
+
+int launch_predict(nb_ctx *ctx, double t)
+{
+    const int64_t N = ctx->N;
+    k_predict<<<(unsigned)((N + 255) / 256), 256, 0, ctx->stream>>>(N, ctx->Npad, t, ctx->t, ctx->mass, ctx->r,
+                                                                    ctx->v, ctx->a, ctx->j, ctx->s, ctx->c,
+                                                                    ctx->jp);
+    NB_LAUNCH_CHECK(ctx, "k_predict");
+    return NB_OK;
+}
+
+// overwrite predicted data from caller-layout arrays (force-only use)
+__global__ void k_set_pred(const int64_t N, const double *__restrict__ pos, const double *__restrict__ vel,
+                           const double *__restrict__ acc, const bool pos_vel, const bool acc_valid,
+                           double *__restrict__ jp)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    double *rec = jp + i * REC;
+    if (pos_vel) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { rec[d] = pos[3 * i + d]; rec[3 + d] = vel[3 * i + d]; }
+    }
+#pragma unroll
+    for (int d = 0; d < 3; ++d) rec[6 + d] = acc_valid ? acc[3 * i + d] : 0.0;
+}
+
+int launch_set_pred(nb_ctx *ctx, const double *pos, const double *vel, const double *acc, bool pos_vel,
+                    bool acc_valid)
+{
+    const int64_t N = ctx->N;
+    k_set_pred<<<(unsigned)((N + 255) / 256), 256, 0, ctx->stream>>>(N, pos, vel, acc, pos_vel, acc_valid, ctx->jp);
+    NB_LAUNCH_CHECK(ctx, "k_set_pred");
+    return NB_OK;
+}
+
+__global__ void k_get_pred(const int64_t N, const double *__restrict__ jp, double *__restrict__ pos,
+                           double *__restrict__ vel, double *__restrict__ acc)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double *rec = jp + i * REC;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        pos[3 * i + d] = rec[d];
+        vel[3 * i + d] = rec[3 + d];
+        acc[3 * i + d] = rec[6 + d];
+    }
+}
+
+int launch_get_pred(nb_ctx *ctx, double *pos, double *vel, double *acc)
+{
+    const int64_t N = ctx->N;
+    k_get_pred<<<(unsigned)((N + 255) / 256), 256, 0, ctx->stream>>>(N, ctx->jp, pos, vel, acc);
+    NB_LAUNCH_CHECK(ctx, "k_get_pred");
+    return NB_OK;
+}
+
+__global__ void k_pack3(const int64_t N, const int64_t Npad, const double *__restrict__ soa,
+                        double *__restrict__ aos)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    aos[3 * i] = soa[i];
+    aos[3 * i + 1] = soa[Npad + i];
+    aos[3 * i + 2] = soa[2 * Npad + i];
+}
+
+int launch_pack3(nb_ctx *ctx, const double *soa, double *aos)
+{
+    const int64_t N = ctx->N;
+    k_pack3<<<(unsigned)((N + 255) / 256), 256, 0, ctx->stream>>>(N, ctx->Npad, soa, aos);
+    NB_LAUNCH_CHECK(ctx, "k_pack3");
+    return NB_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// Next block (Table 1 row 1).  Times are non-negative dyadic rationals, so
+// t_i + dt_i is exact, equality is well defined, and the bit pattern of a non-negative double
+// orders like the value: the minimum is an atomicMin on its 64-bit pattern.
+constexpr int SCHED_THREADS = 256;
+constexpr int SCHED_ITEMS = 8;                        // consecutive particles per thread
+constexpr int SCHED_BLOCK = SCHED_THREADS * SCHED_ITEMS;
+
+__global__ void k_tmin(const int64_t N, const double *__restrict__ t, const double *__restrict__ dt,
+                       unsigned long long *__restrict__ tmin_bits)
+{
+    double v = __longlong_as_double(0x7ff0000000000000LL);
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
+        v = fmin(v, t[i] + dt[i]);
+    for (int off = 16; off > 0; off >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, off));
+    __shared__ double sm[SCHED_THREADS / 32];
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        v = threadIdx.x < SCHED_THREADS / 32 ? sm[threadIdx.x] : __longlong_as_double(0x7ff0000000000000LL);
+        for (int off = 16; off > 0; off >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, off));
+        if (threadIdx.x == 0) atomicMin(tmin_bits, (unsigned long long)__double_as_longlong(v));
+    }
+}
+
+__device__ __forceinline__ int block_exclusive_scan(int v, int *total)
+{
+    // exclusive scan of one int per thread over a SCHED_THREADS-thread block
+    __shared__ int warp_sum[SCHED_THREADS / 32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int incl = v;
+    for (int off = 1; off < 32; off <<= 1) {
+        const int n = __shfl_up_sync(0xffffffffu, incl, off);
+        if (lane >= off) incl += n;
+    }
+    if (lane == 31) warp_sum[w] = incl;
+    __syncthreads();
+    if (w == 0) {
+        int ws = lane < SCHED_THREADS / 32 ? warp_sum[lane] : 0;
+        for (int off = 1; off < 32; off <<= 1) {
+            const int n = __shfl_up_sync(0xffffffffu, ws, off);
+            if (lane >= off) ws += n;
+        }
+        if (lane < SCHED_THREADS / 32) warp_sum[lane] = ws;  // inclusive over warps
+    }
+    __syncthreads();
+    const int base = w ? warp_sum[w - 1] : 0;
+    *total = warp_sum[SCHED_THREADS / 32 - 1];
+    __syncthreads();
+    return base + incl - v;
+}
+
+// per-block match counts; the last block to finish turns them into exclusive offsets and
+// publishes (t_next, n_active) to the pinned host mirror
+__global__ void __launch_bounds__(SCHED_THREADS)
+    k_count_scan(const int64_t N, const double *__restrict__ t, const double *__restrict__ dt,
+                 const unsigned long long *__restrict__ tmin_bits, int32_t *__restrict__ blk_count,
+                 unsigned int *__restrict__ ticket, Sched *__restrict__ sched)
+{
+    const double tn = __longlong_as_double((long long)*tmin_bits);
+    const int64_t base = (int64_t)blockIdx.x * SCHED_BLOCK + (int64_t)threadIdx.x * SCHED_ITEMS;
+    int cnt = 0;
+#pragma unroll
+    for (int u = 0; u < SCHED_ITEMS; ++u) {
+        const int64_t i = base + u;
+        if (i < N && t[i] + dt[i] == tn) ++cnt;
+    }
+    int total;
+    block_exclusive_scan(cnt, &total);
+    __shared__ bool last;
+    if (threadIdx.x == 0) {
+        blk_count[blockIdx.x] = total;
+        __threadfence();
+        const unsigned int tk = atomicAdd(ticket, 1u);
+        last = (tk == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    // exclusive scan of gridDim.x counts by this block, in chunks of SCHED_THREADS
+    int carry = 0;
+    for (int b0 = 0; b0 < (int)gridDim.x; b0 += SCHED_THREADS) {
+        const int b = b0 + threadIdx.x;
+        const int v = b < (int)gridDim.x ? ((volatile int32_t *)blk_count)[b] : 0;
+        int tot;
+        const int ex = block_exclusive_scan(v, &tot);
+        if (b < (int)gridDim.x) blk_count[b] = carry + ex;
+        carry += tot;
+    }
+    if (threadIdx.x == 0) {
+        sched->t_next = tn;
+        sched->n_active = carry;
+        *ticket = 0;
+    }
+}
+
+__global__ void __launch_bounds__(SCHED_THREADS)
+    k_scatter(const int64_t N, const double *__restrict__ t, const double *__restrict__ dt,
+              const unsigned long long *__restrict__ tmin_bits, const int32_t *__restrict__ blk_off,
+              int32_t *__restrict__ active)
+{
+    const double tn = __longlong_as_double((long long)*tmin_bits);
+    const int64_t base = (int64_t)blockIdx.x * SCHED_BLOCK + (int64_t)threadIdx.x * SCHED_ITEMS;
+    bool hit[SCHED_ITEMS];
+    int cnt = 0;
+#pragma unroll
+    for (int u = 0; u < SCHED_ITEMS; ++u) {
+        const int64_t i = base + u;
+        hit[u] = (i < N) && (t[i] + dt[i] == tn);
+        cnt += hit[u] ? 1 : 0;
+    }
+    int total;
+    int pos = blk_off[blockIdx.x] + block_exclusive_scan(cnt, &total);
+#pragma unroll
+    for (int u = 0; u < SCHED_ITEMS; ++u)
+        if (hit[u]) active[pos++] = (int32_t)(base + u);
+}
+
+int launch_next_block(nb_ctx *ctx)
+{
+    const int64_t N = ctx->N;
+    const int nb = (int)ctx->n_sched_blocks;
+    NB_CUDA(ctx, cudaMemsetAsync(ctx->d_tmin, 0x7f, sizeof(unsigned long long), ctx->stream));
+    int g = (int)((N + SCHED_THREADS - 1) / SCHED_THREADS);
+    if (g > 4 * ctx->n_sm) g = 4 * ctx->n_sm;
+    k_tmin<<<g, SCHED_THREADS, 0, ctx->stream>>>(N, ctx->t, ctx->dt, ctx->d_tmin);
+    NB_LAUNCH_CHECK(ctx, "k_tmin");
+    k_count_scan<<<nb, SCHED_THREADS, 0, ctx->stream>>>(N, ctx->t, ctx->dt, ctx->d_tmin, ctx->blk_count,
+                                                        (unsigned int *)(ctx->d_tmin + 1), ctx->d_sched);
+    NB_LAUNCH_CHECK(ctx, "k_count_scan");
+    k_scatter<<<nb, SCHED_THREADS, 0, ctx->stream>>>(N, ctx->t, ctx->dt, ctx->d_tmin, ctx->blk_count, ctx->active);
+    NB_LAUNCH_CHECK(ctx, "k_scatter");
+    return NB_OK;
+}
+
+__global__ void k_tmax(const int64_t N, const double *__restrict__ t, unsigned long long *__restrict__ bits)
+{
+    double v = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
+        v = fmax(v, t[i]);
+    for (int off = 16; off > 0; off >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, off));
+    if ((threadIdx.x & 31) == 0) atomicMax(bits, (unsigned long long)__double_as_longlong(v));
+}
+__global__ void k_publish_t(const unsigned long long *__restrict__ bits, Sched *__restrict__ sched)
+{
+    sched->t_next = __longlong_as_double((long long)*bits);
+    sched->n_active = 0;
+}
+
+int launch_tmax(nb_ctx *ctx)
+{
+    NB_CUDA(ctx, cudaMemsetAsync(ctx->d_tmin, 0, sizeof(unsigned long long), ctx->stream));
+    k_tmax<<<2 * ctx->n_sm, 256, 0, ctx->stream>>>(ctx->N, ctx->t, ctx->d_tmin);
+    NB_LAUNCH_CHECK(ctx, "k_tmax");
+    k_publish_t<<<1, 1, 0, ctx->stream>>>(ctx->d_tmin, ctx->d_sched);
+    NB_LAUNCH_CHECK(ctx, "k_publish_t");
+    return NB_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// Time-step rule, Eq. 15-16 with p = 6 (exponent read as 1/(p-3), G5),
+// quantised to a power of two (G9).  This is an INTEGER decision taken in plain
+// IEEE double, one correctly-rounded operation at a time (the *_rn intrinsics are never
+// contracted into FMAs), in the order the formula is written, so that identical inputs give
+// the identical step:  x = ((eta eta) eta) A1 / A4,  dt_q = 2^floor(ilogb(x)/3),
+// dt = min(dt_q, 2 dt_old); growth only if t_next is a multiple of 2 dt_old; clamp.
+__device__ __forceinline__ double norm3_rn(const double x, const double y, const double z)
+{
+    return __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)), __dmul_rn(z, z)));
+}
+__device__ __forceinline__ double pow2i(int k)  // 2^k for -1022 <= k <= 1023
+{
+    return __longlong_as_double((long long)(k + 1023) << 52);
+}
+__device__ __forceinline__ int ilogb_pos_normal(double x)
+{
+    return (int)((__double_as_longlong(x) >> 52) & 0x7ff) - 1023;
+}
+__device__ __forceinline__ int floordiv3(int e) { return e >= 0 ? e / 3 : -((-e + 2) / 3); }
+
+__device__ double new_dt(const double na, const double nj, const double ns, const double n3,
+                         const double n4, const double n5, const double eta, const double dt_old,
+                         const double t_next, const double dt_min, const double dt_max)
+{
+    const double A1 = __dsqrt_rn(__dadd_rn(__dmul_rn(na, ns), __dmul_rn(nj, nj)));
+    const double A4 = __dsqrt_rn(__dadd_rn(__dmul_rn(n3, n5), __dmul_rn(n4, n4)));
+    double dt_q;
+    if (!(A4 > 0.0)) {
+        dt_q = dt_max;
+    } else {
+        const double x = __ddiv_rn(__dmul_rn(__dmul_rn(__dmul_rn(eta, eta), eta), A1), A4);
+        if (!(x > 0.0)) dt_q = dt_min;
+        else if (isinf(x)) dt_q = dt_max;
+        else if (x < 2.2250738585072014e-308) dt_q = dt_min;  // subnormal: far below any limit
+        else dt_q = pow2i(floordiv3(ilogb_pos_normal(x)));
+    }
+    const double two_old = __dmul_rn(2.0, dt_old);
+    double dt = dt_q < two_old ? dt_q : two_old;
+    if (dt > dt_old) {
+        const double q = __ddiv_rn(t_next, two_old);  // exact: power-of-two divisor
+        if (q != rint(q)) dt = dt_old;
+    }
+    if (dt < dt_min) dt = dt_min;
+    if (dt > dt_max) dt = dt_max;
+    return dt;
+}
+
+// Corrector, Eq. 11-14: v first, r uses the corrected v.  Index 0 = stored
+// values at t_i, index 1 = evaluated at t_i + h.  Then a^(3), a^(4), a^(5) at the END of the
+// step from the quintic Hermite interpolant through (a, jerk, snap) at both ends (G6):
+//   a3 =  3 [20 dA - h ( 8 j0 + 12 j1) + h^2 (3 s1 -   s0)] / h^3
+//   a4 = 12 [30 dA - h (14 j0 + 16 j1) + h^2 (3 s1 - 2 s0)] / h^4
+//   a5 = 60 [12 dA - 6 h (j0 + j1)     + h^2 (  s1 -   s0)] / h^5
+// Commit: r, v <- corrected; a, jerk, snap <- evaluated (G16); crackle <- a3 (G7); t_i <- t_next.
+__global__ void k_correct(const int m, const int64_t Npad, const int32_t *__restrict__ active,
+                          const double t_next, const double eta, const double dt_min, const double dt_max,
+                          const double *__restrict__ f1, double *__restrict__ ti, double *__restrict__ dti,
+                          double *__restrict__ r, double *__restrict__ v, double *__restrict__ a,
+                          double *__restrict__ j, double *__restrict__ s, double *__restrict__ c)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= m) return;
+    const int64_t i = active ? active[k] : k;
+    const double h = dti[i];
+    const double h2 = h * h, h3 = h2 * h;
+    const double ih = 1.0 / h;  // exact: h is a power of two
+    const double ih3 = ih * ih * ih, ih4 = ih3 * ih, ih5 = ih4 * ih;
+    double A1[3], J1[3], S1[3], C3[3], C4[3], C5[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const int64_t q = d * Npad + i;
+        const double r0 = r[q], v0 = v[q], a0 = a[q], j0 = j[q], s0 = s[q];
+        const double a1 = f1[(0 + d) * Npad + k], j1 = f1[(3 + d) * Npad + k], s1 = f1[(6 + d) * Npad + k];
+        const double vc = v0 + (h * 0.5) * (a1 + a0) - (h2 * 0.1) * (j1 - j0) + (h3 * (1.0 / 120.0)) * (s1 + s0);
+        const double rc = r0 + (h * 0.5) * (vc + v0) - (h2 * 0.1) * (a1 - a0) + (h3 * (1.0 / 120.0)) * (j1 + j0);
+        const double dA = a1 - a0;
+        C3[d] = 3.0 * (20.0 * dA - h * (8.0 * j0 + 12.0 * j1) + h2 * (3.0 * s1 - s0)) * ih3;
+        C4[d] = 12.0 * (30.0 * dA - h * (14.0 * j0 + 16.0 * j1) + h2 * (3.0 * s1 - 2.0 * s0)) * ih4;
+        C5[d] = 60.0 * (12.0 * dA - 6.0 * h * (j0 + j1) + h2 * (s1 - s0)) * ih5;
+        A1[d] = a1; J1[d] = j1; S1[d] = s1;
+        r[q] = rc; v[q] = vc; a[q] = a1; j[q] = j1; s[q] = s1; c[q] = C3[d];
+    }
+    ti[i] = t_next;
+    dti[i] = new_dt(norm3_rn(A1[0], A1[1], A1[2]), norm3_rn(J1[0], J1[1], J1[2]), norm3_rn(S1[0], S1[1], S1[2]),
+                    norm3_rn(C3[0], C3[1], C3[2]), norm3_rn(C4[0], C4[1], C4[2]), norm3_rn(C5[0], C5[1], C5[2]),
+                    eta, h, t_next, dt_min, dt_max);
+}
+
+int launch_correct(nb_ctx *ctx, const int32_t *active, int64_t m, double t_next)
+{
+    if (m <= 0) return NB_OK;
+    k_correct<<<(unsigned)((m + 127) / 128), 128, 0, ctx->stream>>>((int)m, ctx->Npad, active, t_next, ctx->eta,
+                                                                    ctx->dt_min, ctx->dt_max, ctx->f1, ctx->t,
+                                                                    ctx->dt, ctx->r, ctx->v, ctx->a, ctx->j,
+                                                                    ctx->s, ctx->c);
+    NB_LAUNCH_CHECK(ctx, "k_correct");
+    return NB_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// Start-up S0 (paper silent; G8).  pass 1: a, jerk <- evaluation with a_pred = 0, and the
+// predicted accelerations become a.  pass 2: a, jerk, snap <- evaluation with a_pred = a;
+// crackle = 0; dt_i = pow2floor(eta_init min(|a|/|jerk|, sqrt(|a|/|snap|))), clamped.
+__global__ void k_startup_commit(const int64_t N, const int64_t Npad, const int pass, const double eta_init,
+                                 const double dt_min, const double dt_max, const double *__restrict__ f1,
+                                 double *__restrict__ a, double *__restrict__ j, double *__restrict__ s,
+                                 double *__restrict__ c, double *__restrict__ ti, double *__restrict__ dti,
+                                 double *__restrict__ jp)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    double A[3], J[3], S[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        A[d] = f1[(0 + d) * Npad + i]; J[d] = f1[(3 + d) * Npad + i]; S[d] = f1[(6 + d) * Npad + i];
+        a[d * Npad + i] = A[d]; j[d * Npad + i] = J[d];
+    }
+    if (pass == 1) {
+        double *rec = jp + i * REC;
+        rec[6] = A[0]; rec[7] = A[1]; rec[8] = A[2];
+        return;
+    }
+#pragma unroll
+    for (int d = 0; d < 3; ++d) { s[d * Npad + i] = S[d]; c[d * Npad + i] = 0.0; }
+    const double na = norm3_rn(A[0], A[1], A[2]), nj = norm3_rn(J[0], J[1], J[2]), ns = norm3_rn(S[0], S[1], S[2]);
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    double q = inf;
+    if (nj > 0.0) q = __ddiv_rn(na, nj);
+    if (ns > 0.0) {
+        const double q2 = __dsqrt_rn(__ddiv_rn(na, ns));
+        if (q2 < q) q = q2;
+    }
+    double dt;
+    if (isinf(q)) dt = dt_max;
+    else {
+        const double x = __dmul_rn(eta_init, q);
+        if (!(x > 0.0) || x < 2.2250738585072014e-308) dt = dt_min;
+        else dt = pow2i(ilogb_pos_normal(x));
+    }
+    if (dt < dt_min) dt = dt_min;
+    if (dt > dt_max) dt = dt_max;
+    ti[i] = 0.0;
+    dti[i] = dt;
+}
+
+int launch_startup_commit(nb_ctx *ctx, int pass)
+{
+    const int64_t N = ctx->N;
+    k_startup_commit<<<(unsigned)((N + 255) / 256), 256, 0, ctx->stream>>>(N, ctx->Npad, pass, ctx->eta_init,
+                                                                           ctx->dt_min, ctx->dt_max, ctx->f1, ctx->a,
+                                                                           ctx->j, ctx->s, ctx->c, ctx->t, ctx->dt,
+                                                                           ctx->jp);
+    NB_LAUNCH_CHECK(ctx, "k_startup_commit");
+    return NB_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// checkpoint: [N][21] = {m, t, dt, r, v, a, jerk, snap, crackle}  <->  SoA planes
+__global__ void k_full_state(const int64_t N, const int64_t Npad, double *__restrict__ st, const bool to_ctx,
+                             double *__restrict__ mass, double *__restrict__ ti, double *__restrict__ dti,
+                             double *__restrict__ r, double *__restrict__ v, double *__restrict__ a,
+                             double *__restrict__ j, double *__restrict__ s, double *__restrict__ c)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    double *p = st + 21 * i;
+    double *planes[6] = {r, v, a, j, s, c};
+    if (to_ctx) {
+        mass[i] = p[0]; ti[i] = p[1]; dti[i] = p[2];
+#pragma unroll
+        for (int q = 0; q < 6; ++q)
+#pragma unroll
+            for (int d = 0; d < 3; ++d) planes[q][d * Npad + i] = p[3 + 3 * q + d];
+    } else {
+        p[0] = mass[i]; p[1] = ti[i]; p[2] = dti[i];
+#pragma unroll
+        for (int q = 0; q < 6; ++q)
+#pragma unroll
+            for (int d = 0; d < 3; ++d) p[3 + 3 * q + d] = planes[q][d * Npad + i];
+    }
+}
+
+int launch_full_state(nb_ctx *ctx, double *state, bool to_ctx)
+{
+    const int64_t N = ctx->N;
+    k_full_state<<<(unsigned)((N + 255) / 256), 256, 0, ctx->stream>>>(N, ctx->Npad, state, to_ctx, ctx->mass, ctx->t,
+                                                                       ctx->dt, ctx->r, ctx->v, ctx->a, ctx->j,
+                                                                       ctx->s, ctx->c);
+    NB_LAUNCH_CHECK(ctx, "k_full_state");
+    return NB_OK;
+}
+
+}  // namespace nb
