@@ -183,6 +183,7 @@ extern "C" int nb_force(nb_ctx *ctx, const int32_t *active_idx, int64_t n_active
     if (!ctx) return NB_EINVAL;
     if (n_active < 0 || n_active > ctx->N) return set_err(ctx, NB_EINVAL, "nb_force: n_active = %lld outside [0, N]", (long long)n_active);
     if (!ctx->pred_valid) return set_err(ctx, NB_ESTATE, "nb_force: no predicted data");
+    if (n_active == 0) { ctx->n_eval = 0; return NB_OK; }  // empty set: nothing to evaluate
     const int32_t *list = nullptr;
     bool sched_set = false;
     if (active_idx) {

@@ -75,6 +75,10 @@ __global__ void __launch_bounds__(EN_THREADS)
     vals[5] = mi * (yi * vz - zi * vy);
     vals[6] = mi * (zi * vx - xi * vz);
     vals[7] = mi * (xi * vy - yi * vx);
+    if (!live) {  // lanes beyond N: their pot may be NaN (eps = 0 against record 0); they own nothing
+#pragma unroll
+        for (int q = 0; q < 8; ++q) vals[q] = 0.0;
+    }
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
         const double tot = block_sum(vals[q], red);
