@@ -9,7 +9,7 @@ steps (a6).  All particles share one time level (dt_min = dt_max), so each step 
 full-N evaluation: N^2 = 1.0995e12 pair interactions.  north_star quotes the metric (FP64 pair
 interactions/s, Tflop/s vs FP64 peak) on this full-N evaluation at N >= 1M.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--n N]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--particles N]
                   [--workload step|force] [--no-cpu-baseline] [--no-e2e]
 
 One JSON line on stdout (rank 0).  `--impl reference` times the CPU oracle (oracle/) on a
@@ -49,7 +49,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--n", type=int, default=1 << 20, help="particles (default 2^20, the configs[2] point north_star names)")
+    ap.add_argument("--particles", dest="n", type=int, default=1 << 20, help="particles (default 2^20, the configs[2] point north_star names)")
     ap.add_argument("--workload", default="step", choices=["step", "force"],
                     help="step: full block step (default); force: nb_force only (profiling aid)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -108,6 +108,22 @@ class ClockSampler:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
         return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
                 "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def max_over_ranks(x: float, world: int, device="cuda") -> float:
+    """MAX over ranks of a per-rank time (torch.distributed; NCCL on GPUs, gloo in the CPU tests)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def whole_job_value(units_per_rank_step: float, steps: int, world: int, ms_max: float) -> float:
+    """Replicas only: every rank processes the same units; value = all ranks' units / max time."""
+    return world * steps * units_per_rank_step / (ms_max * 1e-3)
 
 
 # --------------------------------------------------------------------------------------------
@@ -250,12 +266,9 @@ def run_ours(args):
     launches = nb.nb_get_stats(ctx)["n_launch"] - launches0
     kern_ms = float(np.mean([a.elapsed_time(b) for a, b in force_ms])) if force_ms else float("nan")
     sections = {k: float(np.mean([a.elapsed_time(b) for a, b in v])) for k, v in sect.items() if v}
-    if world > 1:
-        tt = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
+    ms_total = max_over_ranks(ms_total, world)
     pairs_per_step = float(N) * float(N)
-    value = world * K * pairs_per_step / (ms_total * 1e-3)
+    value = whole_job_value(pairs_per_step, K, world, ms_total)
 
     # energy drift over the run as a sanity check that the steps did real work
     diag = {}
@@ -282,11 +295,8 @@ def run_ours(args):
             h_state, h_out = h_out, h_state
         barrier()
         dt = time.perf_counter() - t0
-        if world > 1:
-            tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            dt = float(tt.item())
-        e2e = {"value": world * K * pairs_per_step / dt, "unit": UNIT,
+        dt = max_over_ranks(dt, world)
+        e2e = {"value": whole_job_value(pairs_per_step, K, world, dt * 1e3), "unit": UNIT,
                "h2d_bytes_per_step": int(N * 21 * 8), "d2h_bytes_per_step": int(N * 21 * 8),
                "ms_per_step": dt / K * 1e3,
                "api": "nb_set_full_state(host) -> nb_next_block -> nb_predict -> nb_force -> nb_correct_and_step -> nb_get_full_state(host)"}

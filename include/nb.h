@@ -157,6 +157,15 @@ int nb_get_launch(nb_ctx *ctx, int64_t out[5]);
  * It is the measured denominator quoted beside the nominal FP64 peak. */
 int nb_probe_fp64_peak(nb_ctx *ctx, int64_t iters, double *flops, float *ms);
 
+/* Operand-fetch probe of the FP64 datapath: streams of independent
+ * DFMAs whose source operands are, per mode,
+ *   0: one register + two immediates (pure pipe rate)      1: three distinct registers
+ *   2: three registers, one shared by groups of three consecutive DFMAs (reuse cache)
+ *   3: two distinct registers (a*a + c)
+ * *cycles_per_inst [host] = SM-clock cycles per warp instruction per SM sub-partition, at the
+ * clock `sm_mhz` the caller passes (e.g. the nvidia-smi reading).                          */
+int nb_probe_fp64_operands(nb_ctx *ctx, int mode, int64_t iters, double sm_mhz, double *cycles_per_inst);
+
 const char *nb_last_error(const nb_ctx *ctx);
 void nb_free(nb_ctx *ctx);
 

@@ -159,4 +159,63 @@ int launch_probe(nb_ctx *ctx, int64_t iters, double *flops, float *ms)
     return NB_OK;
 }
 
+// Operand-fetch probe: 12 independent DFMA chains per thread, 24 DFMAs per loop trip, operands
+// pinned by inline PTX so that ptxas cannot fold them.
+template <int MODE>
+__global__ void __launch_bounds__(1024) k_probe_operands(const long long iters, const double seed, double *__restrict__ sink)
+{
+    double x[12], a[12], b[12];
+    const double tf = (double)threadIdx.x;
+#pragma unroll
+    for (int k = 0; k < 12; ++k) {
+        x[k] = seed + k + tf;
+        a[k] = 1.0 + 1e-9 * (k + 1) + tf * 1e-15;
+        b[k] = 1e-9 * (k + 2) + tf * 1e-16;
+    }
+    for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+#pragma unroll
+            for (int k = 0; k < 12; ++k) {
+                if (MODE == 0) asm volatile("fma.rn.f64 %0, %0, 0d3FEFFFFDE7210BE9, 0d3E112E0BE826D695;" : "+d"(x[k]));
+                if (MODE == 1) asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(x[k]) : "d"(a[k]), "d"(b[k]));
+                if (MODE == 2) asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(x[k]) : "d"(a[k / 3]), "d"(b[k]));
+                if (MODE == 3) asm volatile("fma.rn.f64 %0, %1, %1, %0;" : "+d"(x[k]) : "d"(a[k]));
+            }
+        }
+    }
+    double t = 0.0;
+#pragma unroll
+    for (int k = 0; k < 12; ++k) t += x[k];
+    if (t == 123.456) sink[0] = t;
+}
+
+int launch_probe_operands(nb_ctx *ctx, int mode, int64_t iters, double sm_mhz, double *cycles_per_inst)
+{
+    cudaEvent_t e0, e1;
+    NB_CUDA(ctx, cudaEventCreate(&e0));
+    NB_CUDA(ctx, cudaEventCreate(&e1));
+    const int grid = ctx->n_sm, threads = 1024;  // 8 warps per SM sub-partition
+    for (int pass = 0; pass < 2; ++pass) {
+        const long long n = pass ? iters : iters / 8 + 1;
+        if (pass) NB_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
+        switch (mode) {
+            case 0: k_probe_operands<0><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
+            case 1: k_probe_operands<1><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
+            case 2: k_probe_operands<2><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
+            default: k_probe_operands<3><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
+        }
+        NB_LAUNCH_CHECK(ctx, "k_probe_operands");
+    }
+    NB_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
+    NB_CUDA(ctx, cudaEventSynchronize(e1));
+    float t = 0.f;
+    NB_CUDA(ctx, cudaEventElapsedTime(&t, e0, e1));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    const double warp_inst_per_smsp = (double)iters * 24.0 * (threads / 32) / 4.0;
+    if (cycles_per_inst) *cycles_per_inst = (double)t * 1e-3 * sm_mhz * 1e6 / warp_inst_per_smsp;
+    return NB_OK;
+}
+
 }  // namespace nb

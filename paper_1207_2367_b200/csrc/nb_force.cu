@@ -130,7 +130,7 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 // ---- the evaluation kernel -------------------------------------------------------------
 // grid.x: i-blocks, grid.y: j-splits.  JLT = 1: one i per thread.  JLT = 0: JL (runtime,
 // power of two <= 32) consecutive lanes share one i and stride through the tile.
-template <int NT, int TJ, int MINB, int JLT, bool GUARD0>
+template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int UNR = 4>
 __global__ void __launch_bounds__(NT, MINB)
     k_force(const double *__restrict__ jp, const int32_t *__restrict__ active, const int m,
             const int tiles_total, const int tiles_per_split, const int JLr, const double eps2,
@@ -186,7 +186,7 @@ __global__ void __launch_bounds__(NT, MINB)
             Acc9 A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
             const double *q = tile[st];
             if (JLT) {
-#pragma unroll 4
+#pragma unroll UNR
                 for (int jj = 0; jj < TJ; ++jj)
                     pair_body<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
             } else {

@@ -105,6 +105,7 @@ int launch_energy(nb_ctx *ctx, double out_host[9]);
 
 // ----- nb_probe.cu
 int launch_probe(nb_ctx *ctx, int64_t iters, double *flops, float *ms);
+int launch_probe_operands(nb_ctx *ctx, int mode, int64_t iters, double sm_mhz, double *cycles_per_inst);
 
 int set_err(nb_ctx *ctx, int code, const char *fmt, ...);
 

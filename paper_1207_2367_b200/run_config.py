@@ -4,7 +4,7 @@
 
 Inputs are the seeded synthetic recipes of workloads/ (DESIGN.md section 4).  Timing is by CUDA
 events on the context stream (force-only configs) or host wall clock around the device loop
-(integrations), as DESIGN.md section 8 states.  No oracle is involved here.
+(integrations), as DESIGN.md section 8 states.
 """
 from __future__ import annotations
 
@@ -91,9 +91,29 @@ def run_force(nb, cfg, c, Ns, ms_list):
     return {"config": cfg, "name": c["name"], "eps": c["eps"], "rows": rows}
 
 
+def run_probe(nb):
+    """DFMA peak and operand-fetch probes on a tiny context."""
+    import subprocess
+    z = np.zeros((128, 3)); z[:, 0] = np.arange(128)
+    g = nb.NBody(_dev(z), _dev(z), _dev(np.ones(128)), 1e-3, 0.45)
+    try:
+        mhz = float(subprocess.run(["nvidia-smi", "--query-gpu=clocks.max.sm", "--format=csv,noheader,nounits", "-i", "0"],
+                                   capture_output=True, text=True).stdout.split()[0])
+    except Exception:
+        mhz = 1965.0
+    f, ms = nb.nb_probe_fp64_peak(g.ctx, 1 << 17)
+    names = {0: "1 register + immediates", 1: "3 distinct registers", 2: "3 registers, one shared by 3 consecutive DFMAs",
+             3: "2 distinct registers (a*a+c)"}
+    out = {"sm_mhz_assumed": mhz, "dfma_peak_tflops": f / 1e12, "nominal_tflops": PEAK / 1e12,
+           "cycles_per_warp_inst_per_smsp": {names[k]: nb.nb_probe_fp64_operands(g.ctx, k, 20000, mhz) for k in range(4)}}
+    g.close()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--config", type=int, required=True, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=None, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--probe", action="store_true", help="FP64 pipe probes only (DESIGN.md section 6.3)")
     ap.add_argument("--n", type=int, default=None, help="override N (smaller dry runs)")
     ap.add_argument("--t-end", type=float, default=None)
     ap.add_argument("--steps", type=int, default=None)
@@ -101,6 +121,9 @@ def main():
     a = ap.parse_args()
     import paper_1207_2367_b200 as nb
     from workloads import CONFIGS
+    if a.probe or a.config is None:
+        print(json.dumps(run_probe(nb)), flush=True)
+        return
     c = CONFIGS[a.config]
     if c["kind"] == "integrate":
         N = a.n or c["N"]
