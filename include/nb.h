@@ -100,8 +100,11 @@ int nb_force(nb_ctx *ctx, const int32_t *active_idx, int64_t n_active, double *a
 int nb_correct_and_step(nb_ctx *ctx);
 
 /* Block steps (next block, predict, force, correct) repeated while the next block time is
- * <= t_end; identical results to the call sequence.  n_steps [host] (may be NULL) receives
- * the number of block steps taken.  Runs nb_startup first if it has not run.                */
+ * <= t_end; bit-identical results to the call sequence.  n_steps [host] (may be NULL) receives
+ * the number of block steps taken.  Runs nb_startup first if it has not run.  By default the
+ * loop is driven from the device (nb_set_loop_mode): batches of block steps replayed as one
+ * CUDA graph whose kernels read (t_next, n_active) from device memory; the host synchronises
+ * once per batch instead of once per step (Table 1 rows 1, 2, 6, 9 disappear). */
 int nb_run_until(nb_ctx *ctx, double t_end, int64_t *n_steps);
 
 /* Exactly `n` block steps (config 5: "advance 8 block steps").  Optional per-step log
@@ -147,6 +150,11 @@ int nb_get_stats(nb_ctx *ctx, double out[4], int64_t hist[64]);
  * Fig. 8): split = 0 chooses the number of j-splits automatically (default), split >= 1
  * forces it.  jlanes = 0 automatic, else lanes of a warp that share one i (1, 2, 4 .. 32).  */
 int nb_set_tuning(nb_ctx *ctx, int split, int jlanes);
+
+/* Driver of nb_run_until / nb_run_steps: 1 (default) = device-driven CUDA-graph batches,
+ * 0 = the host issues nb_next_block / nb_predict / nb_force / nb_correct_and_step per step.
+ * Both give bit-identical states.  nb_run_steps with a per-step log always uses 0.          */
+int nb_set_loop_mode(nb_ctx *ctx, int device_driven);
 
 /* What the last nb_force launched: out [host] = {threads per CTA, j-lanes per i, j-splits,
  * CTAs, j-tile length}.                                                                     */

@@ -9,6 +9,13 @@
 
 using namespace nb;
 
+static double __longlong_as_double_host(long long b)
+{
+    double d;
+    memcpy(&d, &b, sizeof(d));
+    return d;
+}
+
 static bool is_pow2(double x)
 {
     int e;
@@ -27,6 +34,9 @@ static void release(nb_ctx *ctx)
 {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
+    graph_release(ctx);
+    if (ctx->h_ctl) cudaFreeHost(ctx->h_ctl);
+    if (ctx->ctl) cudaFree(ctx->ctl);
     void *bufs[] = {ctx->mass, ctx->t, ctx->dt, ctx->r, ctx->v, ctx->a, ctx->j, ctx->s, ctx->c, ctx->jp,
                     ctx->active, ctx->user_idx, ctx->f1, ctx->stage, ctx->partials, ctx->d_tmin,
                     ctx->blk_count, ctx->red};
@@ -107,6 +117,10 @@ extern "C" int nb_init(nb_ctx **out, int64_t N, const double *pos, const double 
     if (cudaHostAlloc((void **)&ctx->h_sched, sizeof(Sched), cudaHostAllocMapped) != cudaSuccess) return fail(NB_ENOMEM);
     if (cudaHostGetDevicePointer((void **)&ctx->d_sched, ctx->h_sched, 0) != cudaSuccess) return fail(NB_ECUDA);
     ctx->h_sched->t_next = 0.0; ctx->h_sched->n_active = 0;
+    if ((rc = dev_alloc(ctx, &ctx->ctl, 1))) return fail(rc);
+    if (cudaHostAlloc((void **)&ctx->h_ctl, sizeof(StepCtl), cudaHostAllocDefault) != cudaSuccess) return fail(NB_ENOMEM);
+    memset(ctx->h_ctl, 0, sizeof(StepCtl));
+    ctx->use_graph = 1;
     if ((rc = query_force_occupancy(ctx))) return fail(rc);
 
     // stage the caller's arrays on the device ([N][3] | [N][3] | [N]) and build the SoA state
@@ -242,6 +256,7 @@ extern "C" int nb_run_until(nb_ctx *ctx, double t_end, int64_t *n_steps)
     if (!ctx) return NB_EINVAL;
     if (!isfinite(t_end)) return set_err(ctx, NB_EINVAL, "nb_run_until: bad t_end");
     if (!ctx->started) NB_TRY(nb_startup(ctx));
+    if (ctx->use_graph) return graph_run(ctx, t_end, INT64_MAX, n_steps);
     int64_t n = 0;
     for (;;) {
         if (!ctx->have_block) NB_TRY(nb_next_block(ctx, nullptr, nullptr));
@@ -258,6 +273,10 @@ extern "C" int nb_run_steps(nb_ctx *ctx, int64_t n, double *log_t, int64_t *log_
 {
     if (!ctx || n < 0) return NB_EINVAL;
     if (!ctx->started) NB_TRY(nb_startup(ctx));
+    if (ctx->use_graph && !log_t && !log_m && !log_ms) {
+        if (n == 0) return NB_OK;
+        return graph_run(ctx, __longlong_as_double_host(0x7fefffffffffffffLL), n, nullptr);
+    }
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (log_ms) {
         NB_CUDA(ctx, cudaEventCreate(&e0));
@@ -390,6 +409,14 @@ extern "C" int nb_set_tuning(nb_ctx *ctx, int split, int jlanes)
     if (split < 0 || jlanes < 0 || jlanes > 32 || (jlanes & (jlanes - 1)))
         return set_err(ctx, NB_EINVAL, "nb_set_tuning: split >= 0, jlanes in {0,1,2,4,8,16,32}");
     ctx->force_split = split; ctx->force_jlanes = jlanes;
+    return NB_OK;
+}
+
+extern "C" int nb_set_loop_mode(nb_ctx *ctx, int device_driven)
+{
+    if (!ctx) return NB_EINVAL;
+    if (device_driven != 0 && device_driven != 1) return set_err(ctx, NB_EINVAL, "nb_set_loop_mode: 0 or 1");
+    ctx->use_graph = device_driven;
     return NB_OK;
 }
 

@@ -128,38 +128,32 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 }
 
 // ---- the evaluation kernel -------------------------------------------------------------
-// grid.x: i-blocks, grid.y: j-splits.  JLT = 1: one i per thread.  JLT = 0: JL (runtime,
-// power of two <= 32) consecutive lanes share one i and stride through the tile.
-template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int UNR = 4>
-__global__ void __launch_bounds__(NT, MINB)
-    k_force(const double *__restrict__ jp, const int32_t *__restrict__ active, const int m,
-            const int tiles_total, const int tiles_per_split, const int JLr, const double eps2,
-            double *__restrict__ out, const size_t cstride, const size_t sstride)
+// One work item = (i-block ib, j-split sp): NT/JL i-particles against tiles [sp*tps, sp*tps+nt).
+// JLT = 1: one i per thread.  JLT = 0: JL (runtime, power of two <= 32) consecutive lanes share
+// one i and stride through the tile.  `tc` counts the tiles this CTA has consumed so far: ring
+// stage = tc & 1, mbarrier phase = (tc >> 1) & 1, so the ring carries over from item to item.
+template <int NT, int TJ, int JLT, bool GUARD0, int UNR>
+__device__ __forceinline__ void force_item(const double *__restrict__ jp, const int32_t *__restrict__ active,
+                                           const int m, const int ib, const int sp, const int tiles_total,
+                                           const int tiles_per_split, const int JL, const double eps2,
+                                           double *__restrict__ out, const size_t cstride, const size_t sstride,
+                                           double (*tile)[TJ * REC], uint64_t *full, unsigned &tc)
 {
     constexpr int NS = 2;
     constexpr uint32_t TILE_BYTES = TJ * REC * sizeof(double);
-    __shared__ __align__(128) double tile[NS][TJ * REC];
-    __shared__ __align__(8) uint64_t full[NS];
-
-    const int JL = JLT ? 1 : JLr;
     const int tid = threadIdx.x;
-    const int slots = NT / JL;                      // i-particles per CTA
-    const int k = blockIdx.x * slots + tid / JL;    // slot in the active list
-    const int jl = tid % JL;                        // j-lane
-    const int t0 = blockIdx.y * tiles_per_split;
+    const int slots = NT / JL;              // i-particles per CTA
+    const int k = ib * slots + tid / JL;    // slot in the active list
+    const int jl = tid % JL;                // j-lane
+    const int t0 = sp * tiles_per_split;
     const int nt = min(tiles_per_split, tiles_total - t0);
     const char *src = reinterpret_cast<const char *>(jp) + (size_t)t0 * TILE_BYTES;
 
     if (tid == 0) {
-        mbar_init(&full[0], 1);
-        mbar_init(&full[1], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
-    if (tid == 0) {
         for (int st = 0; st < NS && st < nt; ++st) {
-            mbar_expect_tx(&full[st], TILE_BYTES);
-            bulk_g2s(tile[st], src + (size_t)st * TILE_BYTES, TILE_BYTES, &full[st]);
+            const unsigned sg = (tc + st) & 1u;
+            mbar_expect_tx(&full[sg], TILE_BYTES);
+            bulk_g2s(tile[sg], src + (size_t)st * TILE_BYTES, TILE_BYTES, &full[sg]);
         }
     }
 
@@ -176,15 +170,15 @@ __global__ void __launch_bounds__(NT, MINB)
     const double axi = i3.x, ayi = i3.y, azi = i4;
 
     // a warp whose slots are all beyond m only keeps the barriers company
-    const bool warp_idle = (blockIdx.x * slots + (tid & ~31) / JL) >= m;
+    const bool warp_idle = (ib * slots + (tid & ~31) / JL) >= m;
 
     Acc9 T = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     for (int it = 0; it < nt; ++it) {
-        const int st = it & 1;
-        mbar_wait(&full[st], (it >> 1) & 1);
+        const unsigned sg = tc & 1u;
+        mbar_wait(&full[sg], (tc >> 1) & 1u);
         if (!warp_idle) {
             Acc9 A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
-            const double *q = tile[st];
+            const double *q = tile[sg];
             if (JLT) {
 #pragma unroll UNR
                 for (int jj = 0; jj < TJ; ++jj)
@@ -198,11 +192,12 @@ __global__ void __launch_bounds__(NT, MINB)
             T.jx += A.jx; T.jy += A.jy; T.jz += A.jz;
             T.sx += A.sx; T.sy += A.sy; T.sz += A.sz;
         }
-        __syncthreads();  // every warp is done reading tile[st]
+        __syncthreads();  // every warp is done reading tile[sg]
         if (tid == 0 && it + NS < nt) {
-            mbar_expect_tx(&full[st], TILE_BYTES);
-            bulk_g2s(tile[st], src + (size_t)(it + NS) * TILE_BYTES, TILE_BYTES, &full[st]);
+            mbar_expect_tx(&full[sg], TILE_BYTES);
+            bulk_g2s(tile[sg], src + (size_t)(it + NS) * TILE_BYTES, TILE_BYTES, &full[sg]);
         }
+        ++tc;
     }
 
     if (!JLT) {  // fixed-order butterfly over the JL lanes that share this i
@@ -219,11 +214,64 @@ __global__ void __launch_bounds__(NT, MINB)
         }
     }
     if (k < m && jl == 0) {
-        double *o = out + (size_t)blockIdx.y * sstride + k;
+        double *o = out + (size_t)sp * sstride + k;
         o[0 * cstride] = T.ax; o[1 * cstride] = T.ay; o[2 * cstride] = T.az;
         o[3 * cstride] = T.jx; o[4 * cstride] = T.jy; o[5 * cstride] = T.jz;
         o[6 * cstride] = T.sx; o[7 * cstride] = T.sy; o[8 * cstride] = T.sz;
     }
+}
+
+// grid.x: i-blocks, grid.y: j-splits; geometry passed by the host.
+template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int UNR = 4>
+__global__ void __launch_bounds__(NT, MINB)
+    k_force(const double *__restrict__ jp, const int32_t *__restrict__ active, const int m,
+            const int tiles_total, const int tiles_per_split, const int JLr, const double eps2,
+            double *__restrict__ out, const size_t cstride, const size_t sstride)
+{
+    __shared__ __align__(128) double tile[2][TJ * REC];
+    __shared__ __align__(8) uint64_t full[2];
+    if (threadIdx.x == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    unsigned tc = 0;
+    force_item<NT, TJ, JLT, GUARD0, UNR>(jp, active, m, blockIdx.x, blockIdx.y, tiles_total, tiles_per_split,
+                                         JLT ? 1 : JLr, eps2, out, cstride, sstride, tile, full, tc);
+}
+
+// Persistent form for the device-driven block-step loop (nb_graph.cu): a fixed grid of
+// resident CTAs; the set size and the geometry are read from the control block the scheduler
+// kernel of the same step wrote; CTA b takes the work items b, b + gridDim.x, ...  Item w is
+// (i-block w % n_ib, split w / n_ib), so concurrently running CTAs stream the same j-split.
+template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int UNR = 4>
+__global__ void __launch_bounds__(NT, MINB)
+    k_force_persistent(const double *__restrict__ jp, const int32_t *__restrict__ active_list, const int64_t N,
+                       const int64_t Npad, const double eps2, double *__restrict__ f1,
+                       double *__restrict__ partials, const StepCtl *__restrict__ ctl)
+{
+    if (ctl->done || ctl->g.variant != (JLT ? 0 : 1)) return;
+    __shared__ __align__(128) double tile[2][TJ * REC];
+    __shared__ __align__(8) uint64_t full[2];
+    if (threadIdx.x == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const int m = (int)ctl->n_active;
+    const ForceGeom g = ctl->g;
+    const int32_t *active = (m == N) ? nullptr : active_list;
+    double *out = g.S > 1 ? partials : f1;
+    const size_t cstride = g.S > 1 ? (size_t)g.mpad : (size_t)Npad;
+    const size_t sstride = 9 * (size_t)g.mpad;
+    const int tiles_total = (int)(Npad / TJ);
+    const long long items = (long long)g.n_ib * g.S;
+    unsigned tc = 0;
+    for (long long w = blockIdx.x; w < items; w += gridDim.x)
+        force_item<NT, TJ, JLT, GUARD0, UNR>(jp, active, m, (int)(w % g.n_ib), (int)(w / g.n_ib), tiles_total,
+                                             g.tps, g.JL, eps2, out, cstride, sstride, tile, full, tc);
 }
 
 // ---- partial-sum reduction (Table 1 row 4): f1[c][k] = sum_s part[s][c][k], s ascending ---
@@ -269,9 +317,50 @@ __global__ void k_unpack_f1(const double *__restrict__ f1, const size_t f1stride
     }
 }
 
+// Reduction for the device-driven loop: fixed grid, sizes read from the control block.  Element
+// e = c * m + k; the sum over splits runs in ascending split order exactly as in k_reduce_thread
+// (S < 32) or k_reduce_warp (S >= 32), so both drivers give bit-identical results.
+__global__ void __launch_bounds__(256)
+    k_reduce_persistent(const double *__restrict__ part, const StepCtl *__restrict__ ctl, double *__restrict__ f1,
+                        const size_t f1stride)
+{
+    if (ctl->done || ctl->g.S <= 1) return;
+    const int S = ctl->g.S, m = (int)ctl->n_active;
+    const size_t cstride = (size_t)ctl->g.mpad, sstride = 9 * (size_t)ctl->g.mpad;
+    const long long total = 9LL * m;
+    if (S < 32) {
+        for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
+            const int c = (int)(e / m), k = (int)(e - (long long)c * m);
+            const double *p = part + c * cstride + k;
+            double acc = 0.0;
+            for (int s = 0; s < S; ++s) acc += p[(size_t)s * sstride];
+            f1[c * f1stride + k] = acc;
+        }
+    } else {
+        const int lane = threadIdx.x & 31;
+        const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+        for (long long wid = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; wid < total; wid += nwarps) {
+            const int c = (int)(wid / m), k = (int)(wid - (long long)c * m);
+            const double *p = part + c * cstride + k;
+            double acc = 0.0;
+            for (int s = lane; s < S; s += 32) acc += p[(size_t)s * sstride];
+            for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+            if (lane == 0) f1[c * f1stride + k] = acc;
+        }
+    }
+}
+
 // ---- host side ---------------------------------------------------------------------------
-constexpr int NT_A = 128, TJ_A = 128, MINB_A = 4;   // variant A: one i per thread, m >= 128
-constexpr int NT_B = 32, TJ_B = 64, MINB_B = 16;    // variant B: one warp per CTA, small m
+// The split search never asks for more than MAX_WAVES waves of CTAs, i.e. S * m <= MAX_WAVES x
+// (resident CTAs) x (i-slots per CTA); S <= 65535 splits of mpad <= m + 31 add the slack term.
+static size_t partials_bound(const nb_ctx *ctx)
+{
+    const int64_t a = (int64_t)ctx->n_sm * ctx->occ[0] * NT_A, b = (int64_t)ctx->n_sm * ctx->occ[1] * NT_B;
+    int64_t items = (int64_t)MAX_WAVES * (a > b ? a : b) + 32 * 65536;
+    const int64_t by_n = (ctx->Npad / TJ_B) * (ctx->Npad + 32);   // S <= tiles, mpad <= Npad + 32
+    if (by_n < items) items = by_n;
+    return (size_t)(9 * items);
+}
 
 int query_force_occupancy(nb_ctx *ctx)
 {
@@ -282,30 +371,27 @@ int query_force_occupancy(nb_ctx *ctx)
     NB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
                      &v, k_force<NT_B, TJ_B, MINB_B, 0, false>, NT_B, 0));
     ctx->occ[1] = v > 0 ? v : 1;
+    NB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+                     &v, k_force_persistent<NT_A, TJ_A, MINB_A, 1, false>, NT_A, 0));
+    ctx->occ[2] = v > 0 ? v : 1;
+    NB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+                     &v, k_force_persistent<NT_B, TJ_B, MINB_B, 0, false>, NT_B, 0));
+    ctx->occ[3] = v > 0 ? v : 1;
+    ctx->partials_limit = partials_bound(ctx);
     return NB_OK;
 }
 
-// Number of j-splits.  All CTAs do the same work per tile, so the cost of a launch is
-// waves x (tiles per split + a fixed per-CTA cost `o` in tile units).  For a given number of
-// waves the best S is the largest that still fits, so only those candidates are scored.
-static int choose_split(int64_t n_iblocks, int64_t tiles, int64_t slots, int64_t s_cap)
+int reserve_partials(nb_ctx *ctx, size_t need)
 {
-    if (s_cap > tiles) s_cap = tiles;
-    if (s_cap > 65535) s_cap = 65535;
-    if (s_cap < 1) s_cap = 1;
-    double best = 1e300;
-    int best_s = 1;
-    for (int64_t w = 0; w <= 64; ++w) {
-        int64_t S = (w == 0) ? 1 : (w * slots) / n_iblocks;
-        if (S < 1) continue;
-        if (S > s_cap) S = s_cap;
-        const int64_t tps = (tiles + S - 1) / S;
-        S = (tiles + tps - 1) / tps;  // splits that actually get tiles
-        const int64_t waves = (n_iblocks * S + slots - 1) / slots;
-        const double cost = (double)waves * ((double)tps + 0.75) + 0.002 * (double)S;
-        if (cost < best - 1e-12) { best = cost; best_s = (int)S; }
-    }
-    return best_s;
+    if (need <= ctx->partials_cap) return NB_OK;
+    if (ctx->partials) { NB_CUDA(ctx, cudaStreamSynchronize(ctx->stream)); cudaFree(ctx->partials); }
+    ctx->partials = nullptr; ctx->partials_cap = 0;
+    size_t cap = need + need / 2;
+    if (cap > ctx->partials_limit) cap = ctx->partials_limit;
+    if (cap < need) cap = need;
+    NB_CUDA(ctx, cudaMalloc(&ctx->partials, cap * sizeof(double)));
+    ctx->partials_cap = cap;
+    return NB_OK;
 }
 
 template <int NT, int TJ, int MINB, int JLT>
@@ -323,56 +409,60 @@ static void launch_variant(nb_ctx *ctx, dim3 grid, const int32_t *active, int m,
 int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m)
 {
     if (m <= 0) return NB_OK;
-    const bool varA = (m >= 128) && !(ctx->force_jlanes > 1);
-    int JL = 1;
-    if (!varA) {
-        if (ctx->force_jlanes >= 1) JL = ctx->force_jlanes;
-        else { while (JL < 8 && m * (JL * 2) <= 32) JL *= 2; }
-    }
-    const int NT = varA ? NT_A : NT_B, TJ = varA ? TJ_A : TJ_B;
-    const int64_t slots_per_cta = NT / JL;
-    const int64_t n_ib = (m + slots_per_cta - 1) / slots_per_cta;
+    const ForceGeom g = choose_geom(m, ctx->Npad, ctx->n_sm, ctx->occ[0], ctx->occ[1], (int64_t)ctx->partials_limit,
+                                    ctx->force_split, ctx->force_jlanes);
+    const bool varA = g.variant == 0;
+    const int TJ = varA ? TJ_A : TJ_B;
     const int64_t tiles = ctx->Npad / TJ;
-    const int64_t cta_slots = (int64_t)ctx->n_sm * ctx->occ[varA ? 0 : 1];
-    const int64_t mpad = (m + 31) & ~(int64_t)31;
-    int64_t s_cap = (int64_t)((size_t)1 << 28) / (9 * mpad);  // partials <= 2 GiB
-    int S = ctx->force_split >= 1 ? (int)(ctx->force_split < tiles ? ctx->force_split : tiles)
-                                  : choose_split(n_ib, tiles, cta_slots, s_cap);
-    int64_t tps = (tiles + S - 1) / S;
-    S = (int)((tiles + tps - 1) / tps);
-
     double *out = ctx->f1;
     size_t cstride = (size_t)ctx->Npad, sstride = 0;
-    if (S > 1) {
-        const size_t need = (size_t)S * 9 * (size_t)mpad;
-        if (need > ctx->partials_cap) {
-            if (ctx->partials) { NB_CUDA(ctx, cudaStreamSynchronize(ctx->stream)); cudaFree(ctx->partials); }
-            ctx->partials = nullptr; ctx->partials_cap = 0;
-            size_t cap = need + need / 2;
-            NB_CUDA(ctx, cudaMalloc(&ctx->partials, cap * sizeof(double)));
-            ctx->partials_cap = cap;
-        }
-        out = ctx->partials; cstride = (size_t)mpad; sstride = 9 * (size_t)mpad;
+    if (g.S > 1) {
+        const int rc = reserve_partials(ctx, (size_t)g.S * 9 * (size_t)g.mpad);
+        if (rc != NB_OK) return rc;
+        out = ctx->partials; cstride = (size_t)g.mpad; sstride = 9 * (size_t)g.mpad;
     }
-    dim3 grid((unsigned)n_ib, (unsigned)S, 1);
+    dim3 grid((unsigned)g.n_ib, (unsigned)g.S, 1);
     if (varA)
-        launch_variant<NT_A, TJ_A, MINB_A, 1>(ctx, grid, active, (int)m, (int)tiles, (int)tps, 1, out, cstride, sstride);
+        launch_variant<NT_A, TJ_A, MINB_A, 1>(ctx, grid, active, (int)m, (int)tiles, g.tps, 1, out, cstride, sstride);
     else
-        launch_variant<NT_B, TJ_B, MINB_B, 0>(ctx, grid, active, (int)m, (int)tiles, (int)tps, JL, out, cstride, sstride);
+        launch_variant<NT_B, TJ_B, MINB_B, 0>(ctx, grid, active, (int)m, (int)tiles, g.tps, g.JL, out, cstride, sstride);
     NB_LAUNCH_CHECK(ctx, "k_force");
-    if (S > 1) {
-        if (S < 32) {
-            dim3 g((unsigned)((m + 127) / 128), 9, 1);
-            k_reduce_thread<<<g, 128, 0, ctx->stream>>>(out, S, (int)m, cstride, sstride, ctx->f1, (size_t)ctx->Npad);
+    if (g.S > 1) {
+        if (g.S < 32) {
+            dim3 gr((unsigned)((m + 127) / 128), 9, 1);
+            k_reduce_thread<<<gr, 128, 0, ctx->stream>>>(out, g.S, (int)m, cstride, sstride, ctx->f1, (size_t)ctx->Npad);
         } else {
             const int64_t warps = 9 * m;
-            k_reduce_warp<<<(unsigned)((warps + 7) / 8), 256, 0, ctx->stream>>>(out, S, (int)m, cstride, sstride, ctx->f1, (size_t)ctx->Npad);
+            k_reduce_warp<<<(unsigned)((warps + 7) / 8), 256, 0, ctx->stream>>>(out, g.S, (int)m, cstride, sstride, ctx->f1, (size_t)ctx->Npad);
         }
         NB_LAUNCH_CHECK(ctx, "k_reduce");
     }
-    ctx->last_launch[0] = NT; ctx->last_launch[1] = JL; ctx->last_launch[2] = S;
-    ctx->last_launch[3] = n_ib * S; ctx->last_launch[4] = TJ;
+    ctx->last_launch[0] = varA ? NT_A : NT_B; ctx->last_launch[1] = g.JL; ctx->last_launch[2] = g.S;
+    ctx->last_launch[3] = (int64_t)g.n_ib * g.S; ctx->last_launch[4] = TJ;
     ctx->n_pairs += (double)m * (double)ctx->N;
+    return NB_OK;
+}
+
+// Device-driven loop: both variants are enqueued with fixed grids (one wave of resident CTAs);
+// the one the scheduler kernel did not select returns at once, as does everything when the
+// control block says `done`.  Then the fixed-grid reduction.
+int enqueue_force_persistent(nb_ctx *ctx)
+{
+    const unsigned gA = (unsigned)(ctx->n_sm * ctx->occ[2]), gB = (unsigned)(ctx->n_sm * ctx->occ[3]);
+    if (ctx->eps == 0.0) {
+        k_force_persistent<NT_A, TJ_A, MINB_A, 1, true><<<gA, NT_A, 0, ctx->stream>>>(
+            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);
+        k_force_persistent<NT_B, TJ_B, MINB_B, 0, true><<<gB, NT_B, 0, ctx->stream>>>(
+            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);
+    } else {
+        k_force_persistent<NT_A, TJ_A, MINB_A, 1, false><<<gA, NT_A, 0, ctx->stream>>>(
+            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);
+        k_force_persistent<NT_B, TJ_B, MINB_B, 0, false><<<gB, NT_B, 0, ctx->stream>>>(
+            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);
+    }
+    NB_LAUNCH_CHECK(ctx, "k_force_persistent");
+    k_reduce_persistent<<<(unsigned)(2 * ctx->n_sm), 256, 0, ctx->stream>>>(ctx->partials, ctx->ctl, ctx->f1, (size_t)ctx->Npad);
+    NB_LAUNCH_CHECK(ctx, "k_reduce_persistent");
     return NB_OK;
 }
 

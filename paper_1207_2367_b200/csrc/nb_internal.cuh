@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <limits.h>
 
 #include "../../include/nb.h"
 
@@ -27,6 +28,81 @@ struct Sched {                 // device-written, host-read (pinned, mapped)
     double t_next;
     long long n_active;
 };
+
+// Launch geometry of one evaluation: which kernel variant, how many
+// lanes share one i (JL), how many j-splits (S) of how many tiles each (tps), how many i-blocks.
+struct ForceGeom {
+    int variant;  // 0: variant A (128 threads, one i per thread), 1: variant B (one warp per CTA)
+    int JL, S, tps, n_ib, mpad;
+};
+
+// Control block of the device-resident block-step loop (nb_graph.cu): lives in device memory,
+// written by the kernels of a step, copied to a pinned mirror once per graph launch.
+struct StepCtl {
+    unsigned long long tmin_bits;  // bits of min_i(t_i + dt_i), accumulated for the NEXT block
+    unsigned int ticket;
+    int done;                      // set when the next block lies beyond t_end / no steps left
+    double t_next, t_end, t_now;
+    long long n_active, steps_left, n_steps;
+    double n_pairs;
+    ForceGeom g;
+    long long hist[64];
+};
+
+constexpr int NT_A = 128, TJ_A = 128, MINB_A = 4;   // variant A: one i per thread, m >= 128
+constexpr int NT_B = 32, TJ_B = 64, MINB_B = 16;    // variant B: one warp per CTA, small m
+constexpr int MAX_WAVES = 64;                       // the split search considers 1..MAX_WAVES waves
+
+// Number of j-splits.  All CTAs do the same work per tile, so the cost of a launch is
+// waves x (tiles per split + a fixed per-CTA cost of 0.75 tile) + 0.002 S, in integer
+// thousandths so that host and device take the identical decision.  For a given number of
+// waves the best S is the largest that still fits, so only those candidates are scored.
+__host__ __device__ inline int choose_split(int64_t n_iblocks, int64_t tiles, int64_t slots, int64_t s_cap)
+{
+    if (s_cap > tiles) s_cap = tiles;
+    if (s_cap > 65535) s_cap = 65535;
+    if (s_cap < 1) s_cap = 1;
+    int64_t best = INT64_MAX;
+    int best_s = 1;
+    for (int64_t w = 0; w <= MAX_WAVES; ++w) {
+        int64_t S = (w == 0) ? 1 : (w * slots) / n_iblocks;
+        if (S < 1) continue;
+        if (S > s_cap) S = s_cap;
+        const int64_t tps = (tiles + S - 1) / S;
+        S = (tiles + tps - 1) / tps;  // splits that actually get tiles
+        const int64_t waves = (n_iblocks * S + slots - 1) / slots;
+        const int64_t cost = waves * (tps * 1000 + 750) + 2 * S;
+        if (cost < best) { best = cost; best_s = (int)S; }
+    }
+    return best_s;
+}
+
+// Geometry of the evaluation of m particles against Npad records (host and device).
+__host__ __device__ inline ForceGeom choose_geom(int64_t m, int64_t Npad, int n_sm, int occA, int occB,
+                                                 int64_t partials_cap, int force_split, int force_jlanes)
+{
+    ForceGeom g;
+    const bool varA = (m >= 128) && !(force_jlanes > 1);
+    int JL = 1;
+    if (!varA) {
+        if (force_jlanes >= 1) JL = force_jlanes;
+        else { while (JL < 8 && m * (JL * 2) <= 32) JL *= 2; }
+    }
+    const int NT = varA ? NT_A : NT_B, TJ = varA ? TJ_A : TJ_B;
+    const int64_t slots_per_cta = NT / JL;
+    const int64_t n_ib = (m + slots_per_cta - 1) / slots_per_cta;
+    const int64_t tiles = Npad / TJ;
+    const int64_t cta_slots = (int64_t)n_sm * (varA ? occA : occB);
+    const int64_t mpad = (m + 31) & ~(int64_t)31;
+    const int64_t s_cap = partials_cap / (9 * mpad);
+    int S = force_split >= 1 ? (int)(force_split < tiles ? force_split : tiles)
+                             : choose_split(n_ib, tiles, cta_slots, s_cap);
+    if (S > s_cap) S = (int)(s_cap < 1 ? 1 : s_cap);
+    const int64_t tps = (tiles + S - 1) / S;
+    S = (int)((tiles + tps - 1) / tps);
+    g.variant = varA ? 0 : 1; g.JL = JL; g.S = S; g.tps = (int)tps; g.n_ib = (int)n_ib; g.mpad = (int)mpad;
+    return g;
+}
 
 }  // namespace nb
 
@@ -55,13 +131,21 @@ struct nb_ctx {
     double *f1;                     // [9][Npad]
     double *stage;                  // [9*Npad] staging for [n][3] in/out copies
     double *partials;               // [S][9][mpad]
-    size_t partials_cap;            // in doubles
+    size_t partials_cap;            // in doubles (grown on demand up to partials_limit)
+    size_t partials_limit;          // most the split search can ask for: bounds S in choose_geom
     unsigned long long *d_tmin;     // scheduler scalar: bits of min(t+dt)
     int32_t *blk_count;             // per-block match counts / offsets
     int64_t n_sched_blocks;
     double *red;                    // reduction scratch (energy)
     nb::Sched *h_sched;             // pinned host mirror
     nb::Sched *d_sched;             // device alias of h_sched
+    nb::StepCtl *ctl;               // device control block of the graph-driven block-step loop
+    nb::StepCtl *h_ctl;             // pinned host copy, refreshed after every graph launch
+    cudaGraphExec_t step_graph;     // `graph_batch` block steps captured once per context
+    int graph_batch;
+    int graph_split, graph_jlanes;  // tuning knobs the captured graph was built with
+    int64_t launches_per_batch;     // kernels in one replay of step_graph
+    int use_graph;                  // 1: nb_run_until / nb_run_steps drive the loop from the device
 
     // tuning
     int force_split, force_jlanes;
@@ -85,8 +169,10 @@ namespace nb {
 // arithmetic (the body is the same); it only exists for symmetry of the start-up passes.
 int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m);
 int query_force_occupancy(nb_ctx *ctx);
+int enqueue_force_persistent(nb_ctx *ctx);   // both variants + reduction, geometry read from ctx->ctl
 // f1[c][k] -> out[q][k][3] (q = 0 acc, 1 jerk, 2 snap) contiguous in ctx->stage
 int launch_unpack_f1(nb_ctx *ctx, int64_t m);
+int reserve_partials(nb_ctx *ctx, size_t doubles);
 
 // ----- nb_step.cu
 int launch_load_state(nb_ctx *ctx, const double *pos_dev, const double *vel_dev, const double *mass_dev);
@@ -99,6 +185,14 @@ int launch_correct(nb_ctx *ctx, const int32_t *active, int64_t m, double t_next)
 int launch_startup_commit(nb_ctx *ctx, int pass);                    // pass 1: a,j <- f1 ; pass 2: a,j,s <- f1 + dt
 int launch_full_state(nb_ctx *ctx, double *state, bool to_ctx);
 int launch_tmax(nb_ctx *ctx);                                        // d_sched->t_next = max t_i
+
+int enqueue_graph_step(nb_ctx *ctx);                                 // count/scan, scatter+predict, correct of one step
+int enqueue_graph_correct(nb_ctx *ctx);
+int launch_graph_begin(nb_ctx *ctx, double t_end, int64_t steps);    // seeds ctl (t_end, steps_left, tmin)
+
+// ----- nb_graph.cu
+int graph_run(nb_ctx *ctx, double t_end, int64_t max_steps, int64_t *n_steps);
+void graph_release(nb_ctx *ctx);
 
 // ----- nb_energy.cu
 int launch_energy(nb_ctx *ctx, double out_host[9]);

@@ -48,15 +48,13 @@ int launch_load_state(nb_ctx *ctx, const double *pos, const double *vel, const d
 //   v_p = v + h (a + h/2 (j + h/3 (s + h/4 c)))
 //   a_p = a + h (j + h/2 (s + h/3 c))
 // Reads 19 + 1 doubles, writes one 80-byte record: 240 B per particle.
-__global__ void k_predict(const int64_t N, const int64_t Npad, const double t,
-                          const double *__restrict__ ti, const double *__restrict__ mass,
-                          const double *__restrict__ r, const double *__restrict__ v,
-                          const double *__restrict__ a, const double *__restrict__ j,
-                          const double *__restrict__ s, const double *__restrict__ c,
-                          double *__restrict__ jp)
+__device__ __forceinline__ void predict_one(const int64_t i, const int64_t Npad, const double t,
+                                            const double *__restrict__ ti, const double *__restrict__ mass,
+                                            const double *__restrict__ r, const double *__restrict__ v,
+                                            const double *__restrict__ a, const double *__restrict__ j,
+                                            const double *__restrict__ s, const double *__restrict__ c,
+                                            double *__restrict__ jp)
 {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
     const double h = t - ti[i];
     const double h2 = h * 0.5, h3 = h * (1.0 / 3.0), h4 = h * 0.25, h5 = h * 0.2;
     double rp[3], vp[3], ap[3];
@@ -74,6 +72,18 @@ __global__ void k_predict(const int64_t N, const int64_t Npad, const double t,
     rec[2] = make_double2(vp[1], vp[2]);
     rec[3] = make_double2(ap[0], ap[1]);
     rec[4] = make_double2(ap[2], mass[i]);
+}
+
+__global__ void k_predict(const int64_t N, const int64_t Npad, const double t,
+                          const double *__restrict__ ti, const double *__restrict__ mass,
+                          const double *__restrict__ r, const double *__restrict__ v,
+                          const double *__restrict__ a, const double *__restrict__ j,
+                          const double *__restrict__ s, const double *__restrict__ c,
+                          double *__restrict__ jp)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    predict_one(i, Npad, t, ti, mass, r, v, a, j, s, c, jp);
 }
 
 int launch_predict(nb_ctx *ctx, double t)
@@ -365,15 +375,13 @@ __device__ double new_dt(const double na, const double nj, const double ns, cons
 //   a4 = 12 [30 dA - h (14 j0 + 16 j1) + h^2 (3 s1 - 2 s0)] / h^4
 //   a5 = 60 [12 dA - 6 h (j0 + j1)     + h^2 (  s1 -   s0)] / h^5
 // Commit: r, v <- corrected; a, jerk, snap <- evaluated (G16); crackle <- a3 (G7); t_i <- t_next.
-__global__ void k_correct(const int m, const int64_t Npad, const int32_t *__restrict__ active,
-                          const double t_next, const double eta, const double dt_min, const double dt_max,
-                          const double *__restrict__ f1, double *__restrict__ ti, double *__restrict__ dti,
-                          double *__restrict__ r, double *__restrict__ v, double *__restrict__ a,
-                          double *__restrict__ j, double *__restrict__ s, double *__restrict__ c)
+__device__ __forceinline__ double correct_one(const int k, const int64_t i, const int64_t Npad, const double t_next,
+                                              const double eta, const double dt_min, const double dt_max,
+                                              const double *__restrict__ f1, double *__restrict__ ti,
+                                              double *__restrict__ dti, double *__restrict__ r, double *__restrict__ v,
+                                              double *__restrict__ a, double *__restrict__ j, double *__restrict__ s,
+                                              double *__restrict__ c)
 {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= m) return;
-    const int64_t i = active ? active[k] : k;
     const double h = dti[i];
     const double h2 = h * h, h3 = h2 * h;
     const double ih = 1.0 / h;  // exact: h is a power of two
@@ -394,9 +402,23 @@ __global__ void k_correct(const int m, const int64_t Npad, const int32_t *__rest
         r[q] = rc; v[q] = vc; a[q] = a1; j[q] = j1; s[q] = s1; c[q] = C3[d];
     }
     ti[i] = t_next;
-    dti[i] = new_dt(norm3_rn(A1[0], A1[1], A1[2]), norm3_rn(J1[0], J1[1], J1[2]), norm3_rn(S1[0], S1[1], S1[2]),
-                    norm3_rn(C3[0], C3[1], C3[2]), norm3_rn(C4[0], C4[1], C4[2]), norm3_rn(C5[0], C5[1], C5[2]),
-                    eta, h, t_next, dt_min, dt_max);
+    const double dtn = new_dt(norm3_rn(A1[0], A1[1], A1[2]), norm3_rn(J1[0], J1[1], J1[2]), norm3_rn(S1[0], S1[1], S1[2]),
+                              norm3_rn(C3[0], C3[1], C3[2]), norm3_rn(C4[0], C4[1], C4[2]), norm3_rn(C5[0], C5[1], C5[2]),
+                              eta, h, t_next, dt_min, dt_max);
+    dti[i] = dtn;
+    return t_next + dtn;  // exact: dyadic rationals
+}
+
+__global__ void k_correct(const int m, const int64_t Npad, const int32_t *__restrict__ active,
+                          const double t_next, const double eta, const double dt_min, const double dt_max,
+                          const double *__restrict__ f1, double *__restrict__ ti, double *__restrict__ dti,
+                          double *__restrict__ r, double *__restrict__ v, double *__restrict__ a,
+                          double *__restrict__ j, double *__restrict__ s, double *__restrict__ c)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= m) return;
+    const int64_t i = active ? active[k] : k;
+    correct_one(k, i, Npad, t_next, eta, dt_min, dt_max, f1, ti, dti, r, v, a, j, s, c);
 }
 
 int launch_correct(nb_ctx *ctx, const int32_t *active, int64_t m, double t_next)
@@ -500,6 +522,190 @@ int launch_full_state(nb_ctx *ctx, double *state, bool to_ctx)
                                                                        ctx->dt, ctx->r, ctx->v, ctx->a, ctx->j,
                                                                        ctx->s, ctx->c);
     NB_LAUNCH_CHECK(ctx, "k_full_state");
+    return NB_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// Device-driven block-step loop.  The same steps as above, but every
+// size that depends on the active set is read from the control block StepCtl in device memory,
+// so that the kernels of a step have fixed launch configurations and a batch of steps can be
+// replayed as one CUDA graph without the host learning (t_next, m) in between:
+//   k_g_count            : Table 1 row 1 -- count the due particles per block, scan, publish
+//                          (t_next, m), decide `done`, choose the evaluation geometry
+//   k_g_scatter_predict  : ascending active list + predictor Eq. 3-7 for all N + the part of
+//                          min_i(t_i + dt_i) of the NEXT block that the non-active particles give
+//   (evaluation: k_force_persistent, k_reduce_persistent in nb_force.cu)
+//   k_g_correct          : corrector + new dt for the active set + their part of the next minimum
+__global__ void k_g_begin(StepCtl *ctl, const double t_end, const long long steps)
+{
+    ctl->tmin_bits = 0x7ff0000000000000ULL;
+    ctl->ticket = 0; ctl->done = 0;
+    ctl->t_end = t_end; ctl->steps_left = steps; ctl->n_steps = 0; ctl->n_pairs = 0.0;
+    for (int b = 0; b < 64; ++b) ctl->hist[b] = 0;
+}
+
+__global__ void __launch_bounds__(SCHED_THREADS)
+    k_g_count(const int64_t N, const int64_t Npad, const double *__restrict__ t, const double *__restrict__ dt,
+              int32_t *__restrict__ blk_count, StepCtl *__restrict__ ctl, const int n_sm, const int occA,
+              const int occB, const int64_t partials_limit, const int force_split, const int force_jlanes)
+{
+    const double tn = __longlong_as_double((long long)ctl->tmin_bits);
+    const int64_t base = (int64_t)blockIdx.x * SCHED_BLOCK + (int64_t)threadIdx.x * SCHED_ITEMS;
+    int cnt = 0;
+#pragma unroll
+    for (int u = 0; u < SCHED_ITEMS; ++u) {
+        const int64_t i = base + u;
+        if (i < N && t[i] + dt[i] == tn) ++cnt;
+    }
+    int total;
+    block_exclusive_scan(cnt, &total);
+    __shared__ bool last;
+    if (threadIdx.x == 0) {
+        blk_count[blockIdx.x] = total;
+        __threadfence();
+        const unsigned int tk = atomicAdd(&ctl->ticket, 1u);
+        last = (tk == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    int carry = 0;
+    for (int b0 = 0; b0 < (int)gridDim.x; b0 += SCHED_THREADS) {
+        const int b = b0 + threadIdx.x;
+        const int v = b < (int)gridDim.x ? ((volatile int32_t *)blk_count)[b] : 0;
+        int tot;
+        const int ex = block_exclusive_scan(v, &tot);
+        if (b < (int)gridDim.x) blk_count[b] = carry + ex;
+        carry += tot;
+    }
+    if (threadIdx.x == 0) {
+        ctl->ticket = 0;
+        const bool done = ctl->steps_left <= 0 || !(tn <= ctl->t_end);
+        ctl->done = done ? 1 : 0;
+        if (!done) {
+            const long long m = carry;
+            ctl->t_next = tn;
+            ctl->n_active = m;
+            ctl->g = choose_geom(m, Npad, n_sm, occA, occB, partials_limit, force_split, force_jlanes);
+            ctl->steps_left -= 1;
+            ctl->n_steps += 1;
+            ctl->n_pairs += (double)m * (double)N;
+            int b = 0;
+            while ((1LL << (b + 1)) <= m) ++b;
+            ctl->hist[b] += 1;
+            ctl->tmin_bits = 0x7ff0000000000000ULL;  // every block has read it: start the next minimum
+        }
+    }
+}
+
+__device__ __forceinline__ void block_min_to(double v, unsigned long long *dst)
+{
+    for (int off = 16; off > 0; off >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, off));
+    __shared__ double smin[SCHED_THREADS / 32];
+    if ((threadIdx.x & 31) == 0) smin[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        v = threadIdx.x < (blockDim.x >> 5) ? smin[threadIdx.x] : __longlong_as_double(0x7ff0000000000000LL);
+        for (int off = 16; off > 0; off >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, off));
+        if (threadIdx.x == 0 && v < __longlong_as_double(0x7ff0000000000000LL))
+            atomicMin(dst, (unsigned long long)__double_as_longlong(v));
+    }
+}
+
+__global__ void __launch_bounds__(SCHED_THREADS)
+    k_g_scatter_predict(const int64_t N, const int64_t Npad, const double *__restrict__ t,
+                        const double *__restrict__ dt, const int32_t *__restrict__ blk_off,
+                        int32_t *__restrict__ active, StepCtl *__restrict__ ctl, const double *__restrict__ mass,
+                        const double *__restrict__ r, const double *__restrict__ v, const double *__restrict__ a,
+                        const double *__restrict__ j, const double *__restrict__ s, const double *__restrict__ c,
+                        double *__restrict__ jp)
+{
+    if (ctl->done) return;
+    const double tn = ctl->t_next;
+    const int64_t blk0 = (int64_t)blockIdx.x * SCHED_BLOCK;
+    const int64_t base = blk0 + (int64_t)threadIdx.x * SCHED_ITEMS;
+    bool hit[SCHED_ITEMS];
+    int cnt = 0;
+    double vmin = __longlong_as_double(0x7ff0000000000000LL);
+#pragma unroll
+    for (int u = 0; u < SCHED_ITEMS; ++u) {
+        const int64_t i = base + u;
+        hit[u] = false;
+        if (i < N) {
+            const double due = t[i] + dt[i];
+            hit[u] = (due == tn);
+            if (!hit[u]) vmin = fmin(vmin, due);
+        }
+        cnt += hit[u] ? 1 : 0;
+    }
+    int total;
+    int pos = blk_off[blockIdx.x] + block_exclusive_scan(cnt, &total);
+#pragma unroll
+    for (int u = 0; u < SCHED_ITEMS; ++u)
+        if (hit[u]) active[pos++] = (int32_t)(base + u);
+    // predictor for the same 2048 particles, one per thread and pass (coalesced)
+#pragma unroll 2
+    for (int u = 0; u < SCHED_ITEMS; ++u) {
+        const int64_t i = blk0 + (int64_t)u * SCHED_THREADS + threadIdx.x;
+        if (i < N) predict_one(i, Npad, tn, t, mass, r, v, a, j, s, c, jp);
+    }
+    block_min_to(vmin, &ctl->tmin_bits);
+}
+
+__global__ void __launch_bounds__(SCHED_THREADS)
+    k_g_correct(const int64_t N, const int64_t Npad, const int32_t *__restrict__ active_list,
+                StepCtl *__restrict__ ctl, const double eta, const double dt_min, const double dt_max,
+                const double *__restrict__ f1, double *__restrict__ ti, double *__restrict__ dti,
+                double *__restrict__ r, double *__restrict__ v, double *__restrict__ a, double *__restrict__ j,
+                double *__restrict__ s, double *__restrict__ c)
+{
+    if (ctl->done) return;
+    const int m = (int)ctl->n_active;
+    const double tn = ctl->t_next;
+    const int32_t *active = (m == N) ? nullptr : active_list;
+    double vmin = __longlong_as_double(0x7ff0000000000000LL);
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < m; k += gridDim.x * blockDim.x) {
+        const int64_t i = active ? active[k] : k;
+        vmin = fmin(vmin, correct_one(k, i, Npad, tn, eta, dt_min, dt_max, f1, ti, dti, r, v, a, j, s, c));
+    }
+    block_min_to(vmin, &ctl->tmin_bits);
+    if (blockIdx.x == 0 && threadIdx.x == 0) ctl->t_now = tn;
+}
+
+int launch_graph_begin(nb_ctx *ctx, double t_end, int64_t steps)
+{
+    k_g_begin<<<1, 1, 0, ctx->stream>>>(ctx->ctl, t_end, (long long)steps);
+    NB_LAUNCH_CHECK(ctx, "k_g_begin");
+    int g = (int)((ctx->N + SCHED_THREADS - 1) / SCHED_THREADS);
+    if (g > 4 * ctx->n_sm) g = 4 * ctx->n_sm;
+    k_tmin<<<g, SCHED_THREADS, 0, ctx->stream>>>(ctx->N, ctx->t, ctx->dt, &ctx->ctl->tmin_bits);
+    NB_LAUNCH_CHECK(ctx, "k_tmin");
+    return NB_OK;
+}
+
+int enqueue_graph_step(nb_ctx *ctx)
+{
+    const int nb = (int)ctx->n_sched_blocks;
+    k_g_count<<<nb, SCHED_THREADS, 0, ctx->stream>>>(ctx->N, ctx->Npad, ctx->t, ctx->dt, ctx->blk_count, ctx->ctl,
+                                                      ctx->n_sm, ctx->occ[0], ctx->occ[1],
+                                                      (int64_t)ctx->partials_limit, ctx->force_split,
+                                                      ctx->force_jlanes);
+    NB_LAUNCH_CHECK(ctx, "k_g_count");
+    k_g_scatter_predict<<<nb, SCHED_THREADS, 0, ctx->stream>>>(ctx->N, ctx->Npad, ctx->t, ctx->dt, ctx->blk_count,
+                                                                ctx->active, ctx->ctl, ctx->mass, ctx->r, ctx->v,
+                                                                ctx->a, ctx->j, ctx->s, ctx->c, ctx->jp);
+    NB_LAUNCH_CHECK(ctx, "k_g_scatter_predict");
+    return NB_OK;
+}
+
+int enqueue_graph_correct(nb_ctx *ctx)
+{
+    int64_t g = (ctx->N + SCHED_THREADS - 1) / SCHED_THREADS;
+    if (g > 4 * ctx->n_sm) g = 4 * ctx->n_sm;
+    k_g_correct<<<(unsigned)g, SCHED_THREADS, 0, ctx->stream>>>(ctx->N, ctx->Npad, ctx->active, ctx->ctl, ctx->eta,
+                                                               ctx->dt_min, ctx->dt_max, ctx->f1, ctx->t, ctx->dt,
+                                                               ctx->r, ctx->v, ctx->a, ctx->j, ctx->s, ctx->c);
+    NB_LAUNCH_CHECK(ctx, "k_g_correct");
     return NB_OK;
 }
 
