@@ -51,6 +51,7 @@ struct StepCtl {
 
 constexpr int NT_A = 128, TJ_A = 128, MINB_A = 4;   // variant A: one i per thread, m >= 128
 constexpr int NT_B = 32, TJ_B = 64, MINB_B = 16;    // variant B: one warp per CTA, small m
+constexpr int64_t L2_CHUNK_BYTES = 24 << 20;         // j-stream piece kept L2-resident across i-block waves
 constexpr int MAX_WAVES = 64;                       // the split search considers 1..MAX_WAVES waves
 
 // Number of j-splits.  All CTAs do the same work per tile, so the cost of a launch is
@@ -97,6 +98,14 @@ __host__ __device__ inline ForceGeom choose_geom(int64_t m, int64_t Npad, int n_
     const int64_t s_cap = partials_cap / (9 * mpad);
     int S = force_split >= 1 ? (int)(force_split < tiles ? force_split : tiles)
                              : choose_split(n_ib, tiles, cta_slots, s_cap);
+    if (force_split < 1 && n_ib > cta_slots) {
+        // More than one wave of i-blocks re-reads the whole j-stream once per wave.  Keep the piece
+        // that the concurrently running CTAs stream below L2_CHUNK_BYTES (a cyclic sweep over more
+        // than the L2 of one die misses on every pass), when the partial sums fit.
+        const int64_t tps_max = L2_CHUNK_BYTES / ((int64_t)TJ * REC * 8);
+        const int64_t s_min = (tiles + tps_max - 1) / tps_max;
+        if (s_min > S && s_min <= s_cap) S = (int)s_min;
+    }
     if (S > s_cap) S = (int)(s_cap < 1 ? 1 : s_cap);
     const int64_t tps = (tiles + S - 1) / S;
     S = (int)((tiles + tps - 1) / tps);

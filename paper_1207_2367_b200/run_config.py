@@ -40,18 +40,20 @@ def _timed_force(nb, ctx, idx, n, reps):
     return best
 
 
-def run_integration(nb, cfg, c, N, t_end, n_steps):
+def run_integration(nb, cfg, c, N, t_end, n_steps, loop=None):
     import torch
     from workloads import config_inputs
     pos, vel, m, _ = config_inputs(cfg, N)
     g = nb.NBody(_dev(pos), _dev(vel), _dev(m), c["eps"], c["eta"], dt_min=c["dt_min"], dt_max=c["dt_max"])
+    if loop is not None:
+        nb.nb_set_loop_mode(g.ctx, loop)
     t0 = time.perf_counter(); g.startup(); g.sync(); t_start = time.perf_counter() - t0
     e0 = g.energy()
     out = {"config": cfg, "name": c["name"], "N": N, "eps": c["eps"], "eta": c["eta"],
            "startup_s": t_start, "startup_pairs_per_s": 2.0 * N * N / t_start, "E0": float(e0[0])}
     if n_steps:                                   # config 5: a fixed number of block steps
         lt, lm, ms = g.run_steps(n_steps)
-        out["steps"] = [{"t": float(t), "m": int(mm), "ms": float(x), "pairs_per_s": float(mm) * N / (x * 1e-3)}
+        out["steps"] = [{"t": float(t), "m": int(mm), "ms": float(x), "pairs_per_s": float(mm) * N / (float(x) * 1e-3)}
                         for t, mm, x in zip(lt, lm, ms)]
     else:
         t0 = time.perf_counter(); n = g.run_until(t_end); wall = time.perf_counter() - t0
@@ -91,6 +93,87 @@ def run_force(nb, cfg, c, Ns, ms_list):
     return {"config": cfg, "name": c["name"], "eps": c["eps"], "rows": rows}
 
 
+def run_splitj_sweep(nb, N, ms_list):
+    """SURVEY.md section 8(f) N1 / PAPER.md:256, Fig. 8: evaluation time versus the number m of active
+    particles with the j-split chosen automatically ("Bfactor on") and with one split and one lane
+    per i ("Bfactor off": one thread block per TpB i-particles), same inputs."""
+    import torch
+    from workloads import active_subset, config_inputs
+    pos, vel, m, accp = config_inputs(4, N)
+    g = nb.NBody(_dev(pos), _dev(vel), _dev(m), 1e-4, 0.45)
+    nb.nb_set_pred_acc(g.ctx, _dev(accp))
+    rows = []
+    for mm in ms_list:
+        idx = None if mm == N else _dev(active_subset(N, mm, 40), torch.int32)
+        reps = 0 if mm * N > 4e12 else (1 if mm * N > 5e11 else 3)
+        nb.nb_set_tuning(g.ctx, 0, 0)
+        on = _timed_force(nb, g.ctx, idx, mm, reps)
+        lon = {k: int(v) for k, v in nb.nb_get_launch(g.ctx).items()}
+        nb.nb_set_tuning(g.ctx, 1, 1)
+        off = _timed_force(nb, g.ctx, idx, mm, 0 if mm * N > 1e11 else reps)
+        loff = {k: int(v) for k, v in nb.nb_get_launch(g.ctx).items()}
+        rows.append({"N": N, "m": mm, "ms_split_auto": on, "ms_split_off": off, "gain": off / on,
+                     "pairs_per_s_auto": float(mm) * N / (on * 1e-3), "pairs_per_s_off": float(mm) * N / (off * 1e-3),
+                     "launch_auto": lon, "launch_off": loff})
+        print(json.dumps(rows[-1]), file=sys.stderr, flush=True)
+    g.close()
+    return {"experiment": "splitj_on_off", "rows": rows}
+
+
+def run_heavy(nb, N, frac, t_end, eps=1e-4, eta=0.45):
+    """SURVEY.md 8(f) N1 / PAPER.md:254: Plummer + one heavy particle; small blocks dominate."""
+    from workloads import plummer_with_heavy
+    pos, vel, m = plummer_with_heavy(N, seed=9, heavy_frac=frac)
+    out = {"experiment": "heavy_particle", "N": N, "heavy_frac": frac, "eps": eps, "eta": eta, "t_end": t_end}
+    for mode in (1, 0):
+        g = nb.NBody(_dev(pos), _dev(vel), _dev(m), eps, eta, dt_min=2.0 ** -25, dt_max=2.0 ** -4)
+        nb.nb_set_loop_mode(g.ctx, mode)
+        g.startup(); g.sync()
+        e0 = g.energy()
+        t0 = time.perf_counter(); n = g.run_until(t_end); wall = time.perf_counter() - t0
+        st = g.stats(); e1 = g.energy()
+        pairs = st["n_pairs"] - 2.0 * N * N
+        key = "device_loop" if mode else "host_loop"
+        out[key] = {"block_steps": int(n), "wall_s": wall, "block_step_us": wall / max(n, 1) * 1e6,
+                    "pairs": pairs, "pairs_per_s": pairs / wall, "dE_over_E": float((e1[0] - e0[0]) / e0[0])}
+        if mode:
+            out["active_hist_log2"] = {int(b): int(v) for b, v in enumerate(st["hist"]) if v}
+            _, _, _, dt = g.state()
+            out["dt_levels_log2"] = [int(np.log2(float(dt.min().item()))), int(np.log2(float(dt.max().item())))]
+        g.close()
+    return out
+
+
+def run_fig1(nb, Ns, etas, t_end=4.5, every=0.5, eps=1e-4):
+    """SURVEY.md 8(f) N2 / PAPER.md:136-153 (section 5.1, Eq. 20, Fig. 1) in FP64: mean relative energy and
+    angular-momentum errors over the run, sampled every `every` Henon time units up to t_end = 4.5
+    (9.96 of the paper's time units, G11), versus eta."""
+    from workloads import plummer
+    rows = []
+    for N in Ns:
+        pos, vel, m = plummer(N, seed=1500 + int(np.log2(N)))
+        for eta in etas:
+            g = nb.NBody(_dev(pos), _dev(vel), _dev(m), eps, eta, dt_min=2.0 ** -25, dt_max=2.0 ** -4)
+            g.startup(); g.sync()
+            e0 = g.energy(); L0 = np.linalg.norm(e0[6:9])
+            dE, dL = [], []
+            t0 = time.perf_counter(); steps = 0
+            k = 1
+            while k * every <= t_end + 1e-12:
+                steps += g.run_until(k * every)
+                e = g.energy()
+                dE.append(abs((e[0] - e0[0]) / e0[0])); dL.append(np.linalg.norm(e[6:9] - e0[6:9]) / L0)
+                k += 1
+            wall = time.perf_counter() - t0
+            st = g.stats()
+            rows.append({"N": N, "eta": eta, "mean_dE_over_E": float(np.mean(dE)), "final_dE_over_E": float(dE[-1]),
+                         "mean_dL_over_L": float(np.mean(dL)), "L0": float(L0), "block_steps": int(steps),
+                         "pairs": st["n_pairs"] - 2.0 * N * N, "wall_s": wall})
+            print(json.dumps(rows[-1]), file=sys.stderr, flush=True)
+            g.close()
+    return {"experiment": "fig1_energy_vs_eta", "eps": eps, "t_end": t_end, "sample_every": every, "rows": rows}
+
+
 def run_probe(nb):
     """DFMA peak and operand-fetch probes on a tiny context."""
     import subprocess
@@ -118,9 +201,28 @@ def main():
     ap.add_argument("--t-end", type=float, default=None)
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--max-n", type=int, default=None, help="config 3: largest N of the sweep to run")
+    ap.add_argument("--experiment", default=None, choices=["splitj", "heavy", "fig1"],
+                    help="the 'next' rows of SURVEY.md 8(f): split-j on/off sweep, heavy-particle run, Fig. 1 in FP64")
+    ap.add_argument("--etas", default="0.3,0.45,0.6,0.8,1.0")
+    ap.add_argument("--ns", default=None, help="comma-separated N list for --experiment fig1")
+    ap.add_argument("--heavy-frac", type=float, default=0.05)
+    ap.add_argument("--loop", type=int, default=None, choices=[0, 1], help="0: host-driven loop, 1: device-driven (default)")
     a = ap.parse_args()
     import paper_1207_2367_b200 as nb
     from workloads import CONFIGS
+    if a.experiment == "splitj":
+        N = a.n or (1 << 20)
+        ms = [1, 2, 4, 8, 16, 32, 64, 128, 256, 1024, 4096, 16384, 65536, 262144]
+        print(json.dumps(run_splitj_sweep(nb, N, [x for x in ms if x <= N])), flush=True)
+        return
+    if a.experiment == "heavy":
+        print(json.dumps(run_heavy(nb, a.n or 65536, a.heavy_frac, a.t_end if a.t_end is not None else 0.25)), flush=True)
+        return
+    if a.experiment == "fig1":
+        Ns = [int(x) for x in a.ns.split(",")] if a.ns else [1 << 15]
+        print(json.dumps(run_fig1(nb, Ns, [float(x) for x in a.etas.split(",")],
+                                  t_end=a.t_end if a.t_end is not None else 4.5)), flush=True)
+        return
     if a.probe or a.config is None:
         print(json.dumps(run_probe(nb)), flush=True)
         return
@@ -128,7 +230,8 @@ def main():
     if c["kind"] == "integrate":
         N = a.n or c["N"]
         steps = a.steps if a.steps is not None else c.get("n_block_steps")
-        out = run_integration(nb, a.config, c, N, a.t_end if a.t_end is not None else c.get("t_end"), steps)
+        out = run_integration(nb, a.config, c, N, a.t_end if a.t_end is not None else c.get("t_end"), steps, a.loop)
+        out["loop"] = "host" if a.loop == 0 else "device"
     elif a.config == 3:
         Ns = [a.n] if a.n else [n for n in c["N"] if not a.max_n or n <= a.max_n]
         out = run_force(nb, 3, c, Ns, None)

@@ -6,7 +6,7 @@ inputs shaped like the paper's workloads.
 "Input recipe".
 """
 from .plummer import (CONFIGS, HENON_B, active_subset, config_inputs, kepler_binary,
-                      mean_field_acc, plummer, power_law_masses)
+                      mean_field_acc, plummer, plummer_with_heavy, power_law_masses)
 
 __all__ = ["CONFIGS", "HENON_B", "active_subset", "config_inputs", "kepler_binary",
-           "mean_field_acc", "plummer", "power_law_masses"]
+           "mean_field_acc", "plummer", "plummer_with_heavy", "power_law_masses"]

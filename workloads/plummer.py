@@ -79,6 +79,22 @@ def mean_field_acc(pos: np.ndarray) -> np.ndarray:
     return -pos / (r2 + HENON_B ** 2)[:, None] ** 1.5
 
 
+def plummer_with_heavy(N: int, seed: int, heavy_frac: float = 0.05):
+    """Plummer sphere of N - 1 equal-mass particles plus ONE heavy particle of mass heavy_frac (total
+    mass 1) at rest at the centre: the stand-in for the paper's massive-black-hole runs
+    (initial conditions of its ref. [23] are not available), where the stars bound to
+    the heavy particle take the smallest steps and small blocks dominate the step count."""
+    pos, vel, _ = plummer(N, seed)
+    m = np.full(N, (1.0 - heavy_frac) / (N - 1))
+    m[0] = heavy_frac
+    pos[0] = 0.0
+    vel[0] = 0.0
+    mt = m.sum()
+    pos -= (m[:, None] * pos).sum(axis=0) / mt
+    vel -= (m[:, None] * vel).sum(axis=0) / mt
+    return np.ascontiguousarray(pos), np.ascontiguousarray(vel), m
+
+
 def active_subset(N: int, m: int, seed: int = 40) -> np.ndarray:
     """First m entries of a seeded permutation of 0..N-1 (config 4), as int32."""
     rng = np.random.default_rng(seed)
