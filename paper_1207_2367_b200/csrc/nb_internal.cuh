@@ -57,32 +57,44 @@ constexpr int MAX_WAVES = 64;                       // the split search consider
 // Number of j-splits.  All CTAs do the same work per tile, so the cost of a launch is
 // waves x (tiles per split + a fixed per-CTA cost of 0.75 tile) + 0.002 S, in integer
 // thousandths so that host and device take the identical decision.  For a given number of
-// waves the best S is the largest that still fits, so only those candidates are scored.
-__host__ __device__ inline int choose_split(int64_t n_iblocks, int64_t tiles, int64_t slots, int64_t s_cap)
+// waves w the best S is the largest that still fits, so only the candidates w = 0..MAX_WAVES
+// are scored (w = 0 stands for S = 1); the first candidate with the least cost wins.
+struct SplitProblem {
+    int64_t n_ib, tiles, slots, s_cap;
+};
+// candidate w -> its S; returns the cost, or INT64_MAX when the candidate does not exist
+__host__ __device__ inline int64_t split_candidate(const SplitProblem &p, int64_t w, int *S_out)
 {
-    if (s_cap > tiles) s_cap = tiles;
+    int64_t s_cap = p.s_cap;
+    if (s_cap > p.tiles) s_cap = p.tiles;
     if (s_cap > 65535) s_cap = 65535;
     if (s_cap < 1) s_cap = 1;
+    int64_t S = (w == 0) ? 1 : (w * p.slots) / p.n_ib;
+    if (S < 1) { *S_out = 1; return INT64_MAX; }
+    if (S > s_cap) S = s_cap;
+    const int64_t tps = (p.tiles + S - 1) / S;
+    S = (p.tiles + tps - 1) / tps;  // splits that actually get tiles
+    const int64_t waves = (p.n_ib * S + p.slots - 1) / p.slots;
+    *S_out = (int)S;
+    return waves * (tps * 1000 + 750) + 2 * S;
+}
+__host__ __device__ inline int choose_split(const SplitProblem &p)
+{
     int64_t best = INT64_MAX;
     int best_s = 1;
     for (int64_t w = 0; w <= MAX_WAVES; ++w) {
-        int64_t S = (w == 0) ? 1 : (w * slots) / n_iblocks;
-        if (S < 1) continue;
-        if (S > s_cap) S = s_cap;
-        const int64_t tps = (tiles + S - 1) / S;
-        S = (tiles + tps - 1) / tps;  // splits that actually get tiles
-        const int64_t waves = (n_iblocks * S + slots - 1) / slots;
-        const int64_t cost = waves * (tps * 1000 + 750) + 2 * S;
-        if (cost < best) { best = cost; best_s = (int)S; }
+        int S;
+        const int64_t cost = split_candidate(p, w, &S);
+        if (cost < best) { best = cost; best_s = S; }
     }
     return best_s;
 }
 
-// Geometry of the evaluation of m particles against Npad records (host and device).
-__host__ __device__ inline ForceGeom choose_geom(int64_t m, int64_t Npad, int n_sm, int occA, int occB,
-                                                 int64_t partials_cap, int force_split, int force_jlanes)
+// Geometry of the evaluation of m particles against Npad records, in two halves so that the
+// device can score the split candidates with one thread each (geom_finish takes the winner).
+__host__ __device__ inline SplitProblem geom_begin(ForceGeom &g, int64_t m, int64_t Npad, int n_sm, int occA, int occB,
+                                                   int64_t partials_cap, int force_jlanes)
 {
-    ForceGeom g;
     const bool varA = (m >= 128) && !(force_jlanes > 1);
     int JL = 1;
     if (!varA) {
@@ -91,25 +103,38 @@ __host__ __device__ inline ForceGeom choose_geom(int64_t m, int64_t Npad, int n_
     }
     const int NT = varA ? NT_A : NT_B, TJ = varA ? TJ_A : TJ_B;
     const int64_t slots_per_cta = NT / JL;
-    const int64_t n_ib = (m + slots_per_cta - 1) / slots_per_cta;
-    const int64_t tiles = Npad / TJ;
-    const int64_t cta_slots = (int64_t)n_sm * (varA ? occA : occB);
+    SplitProblem p;
+    p.n_ib = (m + slots_per_cta - 1) / slots_per_cta;
+    p.tiles = Npad / TJ;
+    p.slots = (int64_t)n_sm * (varA ? occA : occB);
     const int64_t mpad = (m + 31) & ~(int64_t)31;
-    const int64_t s_cap = partials_cap / (9 * mpad);
-    int S = force_split >= 1 ? (int)(force_split < tiles ? force_split : tiles)
-                             : choose_split(n_ib, tiles, cta_slots, s_cap);
-    if (force_split < 1 && n_ib > cta_slots) {
+    p.s_cap = partials_cap / (9 * mpad);
+    g.variant = varA ? 0 : 1; g.JL = JL; g.n_ib = (int)p.n_ib; g.mpad = (int)mpad;
+    return p;
+}
+__host__ __device__ inline void geom_finish(ForceGeom &g, const SplitProblem &p, int S_auto, int force_split)
+{
+    const int TJ = g.variant == 0 ? TJ_A : TJ_B;
+    int S = force_split >= 1 ? (int)(force_split < p.tiles ? force_split : p.tiles) : S_auto;
+    if (force_split < 1 && p.n_ib > p.slots) {
         // More than one wave of i-blocks re-reads the whole j-stream once per wave.  Keep the piece
         // that the concurrently running CTAs stream below L2_CHUNK_BYTES (a cyclic sweep over more
         // than the L2 of one die misses on every pass), when the partial sums fit.
         const int64_t tps_max = L2_CHUNK_BYTES / ((int64_t)TJ * REC * 8);
-        const int64_t s_min = (tiles + tps_max - 1) / tps_max;
-        if (s_min > S && s_min <= s_cap) S = (int)s_min;
+        const int64_t s_min = (p.tiles + tps_max - 1) / tps_max;
+        if (s_min > S && s_min <= p.s_cap) S = (int)s_min;
     }
-    if (S > s_cap) S = (int)(s_cap < 1 ? 1 : s_cap);
-    const int64_t tps = (tiles + S - 1) / S;
-    S = (int)((tiles + tps - 1) / tps);
-    g.variant = varA ? 0 : 1; g.JL = JL; g.S = S; g.tps = (int)tps; g.n_ib = (int)n_ib; g.mpad = (int)mpad;
+    if (S > p.s_cap) S = (int)(p.s_cap < 1 ? 1 : p.s_cap);
+    const int64_t tps = (p.tiles + S - 1) / S;
+    S = (int)((p.tiles + tps - 1) / tps);
+    g.S = S; g.tps = (int)tps;
+}
+__host__ __device__ inline ForceGeom choose_geom(int64_t m, int64_t Npad, int n_sm, int occA, int occB,
+                                                 int64_t partials_cap, int force_split, int force_jlanes)
+{
+    ForceGeom g;
+    const SplitProblem p = geom_begin(g, m, Npad, n_sm, occA, occB, partials_cap, force_jlanes);
+    geom_finish(g, p, force_split >= 1 ? 1 : choose_split(p), force_split);
     return g;
 }
 

@@ -578,23 +578,45 @@ __global__ void __launch_bounds__(SCHED_THREADS)
         if (b < (int)gridDim.x) blk_count[b] = carry + ex;
         carry += tot;
     }
+    // the last block decides: done?, (t_next, m), and the evaluation geometry.  The split
+    // candidates (choose_split's loop) are scored by one thread each: 65 x a few 64-bit divisions
+    // in a single thread would cost more than the rest of the step.
+    __shared__ ForceGeom sg;
+    __shared__ SplitProblem sp;
+    __shared__ long long scost[MAX_WAVES + 1];
+    __shared__ int ssplit[MAX_WAVES + 1];
+    __shared__ int sdone;
+    const long long m = carry;
     if (threadIdx.x == 0) {
         ctl->ticket = 0;
-        const bool done = ctl->steps_left <= 0 || !(tn <= ctl->t_end);
-        ctl->done = done ? 1 : 0;
-        if (!done) {
-            const long long m = carry;
-            ctl->t_next = tn;
-            ctl->n_active = m;
-            ctl->g = choose_geom(m, Npad, n_sm, occA, occB, partials_limit, force_split, force_jlanes);
-            ctl->steps_left -= 1;
-            ctl->n_steps += 1;
-            ctl->n_pairs += (double)m * (double)N;
-            int b = 0;
-            while ((1LL << (b + 1)) <= m) ++b;
-            ctl->hist[b] += 1;
-            ctl->tmin_bits = 0x7ff0000000000000ULL;  // every block has read it: start the next minimum
-        }
+        sdone = (ctl->steps_left <= 0 || !(tn <= ctl->t_end)) ? 1 : 0;
+        ctl->done = sdone;
+        if (!sdone) sp = geom_begin(sg, m, Npad, n_sm, occA, occB, partials_limit, force_jlanes);
+    }
+    __syncthreads();
+    if (sdone) return;
+    if (threadIdx.x <= MAX_WAVES) {
+        int S;
+        scost[threadIdx.x] = split_candidate(sp, threadIdx.x, &S);
+        ssplit[threadIdx.x] = S;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        long long best = INT64_MAX;
+        int best_s = 1;
+        for (int w = 0; w <= MAX_WAVES; ++w)
+            if (scost[w] < best) { best = scost[w]; best_s = ssplit[w]; }
+        geom_finish(sg, sp, best_s, force_split);
+        ctl->t_next = tn;
+        ctl->n_active = m;
+        ctl->g = sg;
+        ctl->steps_left -= 1;
+        ctl->n_steps += 1;
+        ctl->n_pairs += (double)m * (double)N;
+        int b = 0;
+        while ((1LL << (b + 1)) <= m) ++b;
+        ctl->hist[b] += 1;
+        ctl->tmin_bits = 0x7ff0000000000000ULL;  // every block has read it: start the next minimum
     }
 }
 
@@ -613,7 +635,7 @@ __device__ __forceinline__ void block_min_to(double v, unsigned long long *dst)
 }
 
 __global__ void __launch_bounds__(SCHED_THREADS)
-    k_g_scatter_predict(const int64_t N, const int64_t Npad, const double *__restrict__ t,
+    k_g_scatter_predict(const int64_t N, const int64_t Npad, const int n_sched_blocks, const double *__restrict__ t,
                         const double *__restrict__ dt, const int32_t *__restrict__ blk_off,
                         int32_t *__restrict__ active, StepCtl *__restrict__ ctl, const double *__restrict__ mass,
                         const double *__restrict__ r, const double *__restrict__ v, const double *__restrict__ a,
@@ -622,8 +644,14 @@ __global__ void __launch_bounds__(SCHED_THREADS)
 {
     if (ctl->done) return;
     const double tn = ctl->t_next;
-    const int64_t blk0 = (int64_t)blockIdx.x * SCHED_BLOCK;
-    const int64_t base = blk0 + (int64_t)threadIdx.x * SCHED_ITEMS;
+    // predictor: one particle per thread (coalesced), grid = ceil(N / 256) blocks
+    {
+        const int64_t i = (int64_t)blockIdx.x * SCHED_THREADS + threadIdx.x;
+        if (i < N) predict_one(i, Npad, tn, t, mass, r, v, a, j, s, c, jp);
+    }
+    // the first n_sched_blocks blocks also gather the active list of their 2048-particle chunk
+    if (blockIdx.x >= n_sched_blocks) return;
+    const int64_t base = (int64_t)blockIdx.x * SCHED_BLOCK + (int64_t)threadIdx.x * SCHED_ITEMS;
     bool hit[SCHED_ITEMS];
     int cnt = 0;
     double vmin = __longlong_as_double(0x7ff0000000000000LL);
@@ -643,12 +671,6 @@ __global__ void __launch_bounds__(SCHED_THREADS)
 #pragma unroll
     for (int u = 0; u < SCHED_ITEMS; ++u)
         if (hit[u]) active[pos++] = (int32_t)(base + u);
-    // predictor for the same 2048 particles, one per thread and pass (coalesced)
-#pragma unroll 2
-    for (int u = 0; u < SCHED_ITEMS; ++u) {
-        const int64_t i = blk0 + (int64_t)u * SCHED_THREADS + threadIdx.x;
-        if (i < N) predict_one(i, Npad, tn, t, mass, r, v, a, j, s, c, jp);
-    }
     block_min_to(vmin, &ctl->tmin_bits);
 }
 
@@ -691,7 +713,8 @@ int enqueue_graph_step(nb_ctx *ctx)
                                                       (int64_t)ctx->partials_limit, ctx->force_split,
                                                       ctx->force_jlanes);
     NB_LAUNCH_CHECK(ctx, "k_g_count");
-    k_g_scatter_predict<<<nb, SCHED_THREADS, 0, ctx->stream>>>(ctx->N, ctx->Npad, ctx->t, ctx->dt, ctx->blk_count,
+    const unsigned np = (unsigned)((ctx->N + SCHED_THREADS - 1) / SCHED_THREADS);
+    k_g_scatter_predict<<<np, SCHED_THREADS, 0, ctx->stream>>>(ctx->N, ctx->Npad, nb, ctx->t, ctx->dt, ctx->blk_count,
                                                                 ctx->active, ctx->ctl, ctx->mass, ctx->r, ctx->v,
                                                                 ctx->a, ctx->j, ctx->s, ctx->c, ctx->jp);
     NB_LAUNCH_CHECK(ctx, "k_g_scatter_predict");
