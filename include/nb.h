@@ -170,6 +170,10 @@ int nb_probe_fp64_peak(nb_ctx *ctx, int64_t iters, double *flops, float *ms);
  *   0: one register + two immediates (pure pipe rate)      1: three distinct registers
  *   2: three registers, one shared by groups of three consecutive DFMAs (reuse cache)
  *   3: two distinct registers (a*a + c)
+ *   4: three registers, the first shared by ALL DFMAs (reuse-cache hit on every instruction but
+ *      the one after each scheduler yield)
+ *   5: alternating 3-register DFMA and a DADD that shares one source with it (1 fresh read)
+ *   6: alternating 3-register DFMA and a DADD with its own sources (2 fresh reads)
  * *cycles_per_inst [host] = SM-clock cycles per warp instruction per SM sub-partition, at the
  * clock `sm_mhz` the caller passes (e.g. the nvidia-smi reading).                          */
 int nb_probe_fp64_operands(nb_ctx *ctx, int mode, int64_t iters, double sm_mhz, double *cycles_per_inst);

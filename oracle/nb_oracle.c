@@ -10,6 +10,7 @@
  * computes, written from PAPER.md, one function per passage:
  *
  *   orc_force            Eq. 8-10 with the Eq. 2 softening
+ *   orc_force_mixed      the same in the paper's mixed precision (reading G27)
  *   orc_predict          Eq. 3-7
  *   orc_correct_particle Eq. 11-14 + end-point derivatives of the
  *                        quintic Hermite interpolant (reading G6)
@@ -98,6 +99,64 @@ void orc_force(int64_t N, const double *rp, const double *vp, const double *ap,
             if (acc) acc[3 * k + d] = (double)A0[d];
             if (jerk) jerk[3 * k + d] = (double)A1[d];
             if (snap) snap[3 * k + d] = (double)A2[d];
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------ */
+/* Evaluation step in the paper's MIXED precision (section 5.7: "store predicted
+ * positions, accelerations and derivatives [in double], while it computes partial results in
+ * single precision mode using 32 bit registers"; 15 DP + 82 SP operations per pair,
+ * PAPER.md:301).  Reading G27: the nine differences r_ij, v_ij, a_ij are formed in
+ * double from the double predicted data and rounded to float; everything of Eq. 8-10 for the
+ * pair (r^2 + eps^2, r^3, alpha, beta, the three pair terms) is float arithmetic, one rounded
+ * operation at a time in the order written; the pair terms are summed over j in long double
+ * (so that the sum itself adds no error: what is measured is the SP pair arithmetic).
+ * scale (may be NULL) [n_idx][3] receives sum_j |pair term|_2 for acc, jerk, snap: the
+ * magnitude any forward error bound of a float evaluation is relative to.              */
+void orc_force_mixed(int64_t N, const double *rp, const double *vp, const double *ap,
+                     const double *mass, double eps, const int32_t *idx, int64_t n_idx,
+                     double *acc, double *jerk, double *snap, double *scale)
+{
+    const float eps2 = (float)eps * (float)eps;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t k = 0; k < n_idx; ++k) {
+        const int64_t i = idx ? (int64_t)idx[k] : k;
+        ld A0[3] = {0, 0, 0}, A1[3] = {0, 0, 0}, A2[3] = {0, 0, 0}, sc[3] = {0, 0, 0};
+        for (int64_t j = 0; j < N; ++j) {
+            if (j == i) continue;
+            float r[3], v[3], a[3];
+            for (int d = 0; d < 3; ++d) {
+                r[d] = (float)(rp[3 * j + d] - rp[3 * i + d]); /* DP difference, then SP */
+                v[d] = (float)(vp[3 * j + d] - vp[3 * i + d]);
+                a[d] = (float)(ap[3 * j + d] - ap[3 * i + d]);
+            }
+            const float s = r[0] * r[0] + r[1] * r[1] + r[2] * r[2] + eps2;
+            const float r3 = s * sqrtf(s);
+            const float rv = r[0] * v[0] + r[1] * v[1] + r[2] * v[2];
+            const float vv = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+            const float ra = r[0] * a[0] + r[1] * a[1] + r[2] * a[2];
+            const float alpha = rv / s;
+            const float beta = (vv + ra) / s + alpha * alpha;
+            const float mj = (float)mass[j];
+            float t0[3], t1[3], t2[3];
+            for (int d = 0; d < 3; ++d) {
+                t0[d] = mj * r[d] / r3;                                       /* Eq. 8  */
+                t1[d] = mj * v[d] / r3 - 3.0f * alpha * t0[d];                /* Eq. 9  */
+                t2[d] = mj * a[d] / r3 - 6.0f * alpha * t1[d] - 3.0f * beta * t0[d]; /* Eq. 10 */
+                A0[d] += (ld)t0[d];
+                A1[d] += (ld)t1[d];
+                A2[d] += (ld)t2[d];
+            }
+            sc[0] += sqrtl((ld)t0[0] * t0[0] + (ld)t0[1] * t0[1] + (ld)t0[2] * t0[2]);
+            sc[1] += sqrtl((ld)t1[0] * t1[0] + (ld)t1[1] * t1[1] + (ld)t1[2] * t1[2]);
+            sc[2] += sqrtl((ld)t2[0] * t2[0] + (ld)t2[1] * t2[1] + (ld)t2[2] * t2[2]);
+        }
+        for (int d = 0; d < 3; ++d) {
+            if (acc) acc[3 * k + d] = (double)A0[d];
+            if (jerk) jerk[3 * k + d] = (double)A1[d];
+            if (snap) snap[3 * k + d] = (double)A2[d];
+            if (scale) scale[3 * k + d] = (double)sc[d];
         }
     }
 }

@@ -49,6 +49,7 @@ def lib():
     if _lib is None:
         L = C.CDLL(build())
         L.orc_force.argtypes = [C.c_int64, _dp, _dp, _dp, _dp, C.c_double, _ip, C.c_int64, _dp, _dp, _dp]
+        L.orc_force_mixed.argtypes = [C.c_int64, _dp, _dp, _dp, _dp, C.c_double, _ip, C.c_int64, _dp, _dp, _dp, _dp]
         L.orc_predict.argtypes = [C.c_int64, C.c_double] + [_dp] * 10
         L.orc_correct_particle.argtypes = [C.c_double] + [_dp] * 13
         L.orc_timestep.argtypes = [_dp] * 6 + [C.c_double] * 5
@@ -104,6 +105,22 @@ def force(pos_pred, vel_pred, acc_pred, mass, eps, idx=None):
     acc = np.zeros((n, 3)); jerk = np.zeros((n, 3)); snap = np.zeros((n, 3))
     lib().orc_force(N, _d(rp), _d(vp), _d(ap), _d(m), float(eps), ip, n, _d(acc), _d(jerk), _d(snap))
     return acc, jerk, snap
+
+
+def force_mixed(pos_pred, vel_pred, acc_pred, mass, eps, idx=None):
+    """Eq. 8-10 in the paper's mixed precision (reading G27): DP differences, SP pair
+    arithmetic.  Returns (acc, jerk, snap, scale), scale[k] = sum_j |pair term|_2 per quantity."""
+    rp, vp, ap = _arr(pos_pred), _arr(vel_pred), _arr(acc_pred)
+    m = _arr(mass)
+    N = m.shape[0]
+    if idx is None:
+        n, ip = N, None
+    else:
+        idx = np.ascontiguousarray(idx, dtype=np.int32)
+        n, ip = idx.shape[0], idx.ctypes.data_as(_ip)
+    acc = np.zeros((n, 3)); jerk = np.zeros((n, 3)); snap = np.zeros((n, 3)); scale = np.zeros((n, 3))
+    lib().orc_force_mixed(N, _d(rp), _d(vp), _d(ap), _d(m), float(eps), ip, n, _d(acc), _d(jerk), _d(snap), _d(scale))
+    return acc, jerk, snap, scale
 
 
 def predict(t, ti, r, v, a, j, s, c):

@@ -435,6 +435,6 @@ extern "C" int nb_probe_fp64_peak(nb_ctx *ctx, int64_t iters, double *flops, flo
 
 extern "C" int nb_probe_fp64_operands(nb_ctx *ctx, int mode, int64_t iters, double sm_mhz, double *cycles_per_inst)
 {
-    if (!ctx || iters < 1 || mode < 0 || mode > 3 || !(sm_mhz > 0.0)) return NB_EINVAL;
+    if (!ctx || iters < 1 || mode < 0 || mode > 6 || !(sm_mhz > 0.0)) return NB_EINVAL;
     return launch_probe_operands(ctx, mode, iters, sm_mhz, cycles_per_inst);
 }

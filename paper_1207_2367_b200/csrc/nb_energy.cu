@@ -162,15 +162,16 @@ int launch_probe(nb_ctx *ctx, int64_t iters, double *flops, float *ms)
 // Operand-fetch probe: 12 independent DFMA chains per thread, 24 DFMAs per loop trip, operands
 // pinned by inline PTX so that ptxas cannot fold them.
 template <int MODE>
-__global__ void __launch_bounds__(1024) k_probe_operands(const long long iters, const double seed, double *__restrict__ sink)
+__global__ void __launch_bounds__(512) k_probe_operands(const long long iters, const double seed, double *__restrict__ sink)
 {
     double x[12], a[12], b[12];
     const double tf = (double)threadIdx.x;
 #pragma unroll
     for (int k = 0; k < 12; ++k) {
         x[k] = seed + k + tf;
-        a[k] = 1.0 + 1e-9 * (k + 1) + tf * 1e-15;
-        b[k] = 1e-9 * (k + 2) + tf * 1e-16;
+        // loaded, not computed: ptxas would otherwise re-materialise them inside the timed loop
+        a[k] = sink[1 + k] + tf * 1e-15;
+        b[k] = sink[13 + k] + tf * 1e-16;
     }
     for (long long it = 0; it < iters; ++it) {
 #pragma unroll
@@ -181,6 +182,15 @@ __global__ void __launch_bounds__(1024) k_probe_operands(const long long iters, 
                 if (MODE == 1) asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(x[k]) : "d"(a[k]), "d"(b[k]));
                 if (MODE == 2) asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(x[k]) : "d"(a[k / 3]), "d"(b[k]));
                 if (MODE == 3) asm volatile("fma.rn.f64 %0, %1, %1, %0;" : "+d"(x[k]) : "d"(a[k]));
+                if (MODE == 4) asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(x[k]) : "d"(a[0]), "d"(b[k]));
+                if (MODE == 5) {  // 3-register DFMA, then a DADD that shares one operand with it (1 fresh read)
+                    if (k % 2 == 0) asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(x[k]) : "d"(a[k]), "d"(b[k]));
+                    else asm volatile("add.f64 %0, %1, %0;" : "+d"(x[k]) : "d"(a[k - 1]));
+                }
+                if (MODE == 6) {  // 3-register DFMA, then a DADD with its own second operand (2 fresh reads)
+                    if (k % 2 == 0) asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(x[k]) : "d"(a[k]), "d"(b[k]));
+                    else asm volatile("add.f64 %0, %1, %0;" : "+d"(x[k]) : "d"(b[k]));
+                }
             }
         }
     }
@@ -195,7 +205,7 @@ int launch_probe_operands(nb_ctx *ctx, int mode, int64_t iters, double sm_mhz, d
     cudaEvent_t e0, e1;
     NB_CUDA(ctx, cudaEventCreate(&e0));
     NB_CUDA(ctx, cudaEventCreate(&e1));
-    const int grid = ctx->n_sm, threads = 1024;  // 8 warps per SM sub-partition
+    const int grid = ctx->n_sm, threads = 512;  // 4 warps per SM sub-partition, as in the evaluation kernel
     for (int pass = 0; pass < 2; ++pass) {
         const long long n = pass ? iters : iters / 8 + 1;
         if (pass) NB_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
@@ -203,7 +213,10 @@ int launch_probe_operands(nb_ctx *ctx, int mode, int64_t iters, double sm_mhz, d
             case 0: k_probe_operands<0><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
             case 1: k_probe_operands<1><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
             case 2: k_probe_operands<2><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
-            default: k_probe_operands<3><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
+            case 3: k_probe_operands<3><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
+            case 4: k_probe_operands<4><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
+            case 5: k_probe_operands<5><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
+            default: k_probe_operands<6><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
         }
         NB_LAUNCH_CHECK(ctx, "k_probe_operands");
     }

@@ -115,3 +115,35 @@ def test_self_term_is_skipped_and_N1_is_zero(oracle):
     z = np.zeros((1, 3))
     acc, jerk, snap = oracle.force(z + 1.0, z + 2.0, z + 3.0, np.array([5.0]), 0.0)
     assert np.all(acc == 0) and np.all(jerk == 0) and np.all(snap == 0)
+
+
+# ---- the mixed-precision restatement (orc_force_mixed, reading G27) -----------
+def test_mixed_oracle_is_the_fp64_result_to_single_precision(oracle):
+    """Pinned to the (already pinned) FP64 evaluation: the same sums to a few float ulps of
+    sum_j |pair term| -- and NOT better than that, i.e. the pair arithmetic really is SP."""
+    pos, vel, m = plummer(1500, seed=14)
+    rng = np.random.default_rng(6)
+    ap = rng.normal(size=pos.shape)
+    ref = oracle.force(pos, vel, ap, m, 1e-3)
+    a, j, s, scale = oracle.force_mixed(pos, vel, ap, m, 1e-3)
+    u = 2.0 ** -24
+    for q, (x, y) in enumerate(zip(ref, (a, j, s))):
+        err = np.abs(x - y).max(axis=1) / scale[:, q]
+        assert err.max() <= 16 * u, (q, err.max())          # forward error of ~10 float operations
+        assert np.median(err) >= 1e-3 * u                    # not a double evaluation in disguise
+    # scale is what it says: sum_j |pair term|, >= |sum|
+    for q, x in enumerate(ref):
+        assert np.all(scale[:, q] >= np.linalg.norm(x, axis=1) * (1 - 1e-6))
+
+
+def test_mixed_oracle_two_body_closed_form(oracle):
+    # a = m2 d / (d^2 + eps^2)^(3/2) along x, to float precision; the DP difference keeps a small
+    # separation exact even far from the origin (the reason the paper differences in DP)
+    for x0 in (0.0, 1.0e4):
+        d, eps = 3.0e-3, 1.0e-3
+        pos = np.array([[x0, 0.0, 0.0], [x0 + d, 0.0, 0.0]])
+        z = np.zeros((2, 3))
+        a, j, s, _ = oracle.force_mixed(pos, z, z, np.array([0.25, 0.75]), eps)
+        exact = 0.75 * d / (d * d + eps * eps) ** 1.5
+        assert abs(a[0, 0] - exact) <= 4 * 2.0 ** -24 * exact
+        assert np.all(j == 0) and np.all(s == 0) and a[0, 1] == 0 and a[0, 2] == 0
