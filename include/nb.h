@@ -13,7 +13,8 @@
  *   power-of-two time steps (Eq. 15-16).  Diagnostics: Eq. 20.
  *
  * Conventions
- *   - All arithmetic is IEEE binary64.  Every step runs in CUDA kernels on the device the
+ *   - All arithmetic is IEEE binary64 (unless nb_set_precision selects the paper's mixed
+ *     evaluation).  Every step runs in CUDA kernels on the device the
  *     context was created on; there is no CPU fallback.  A call made without a usable
  *     CUDA device fails with NB_ECUDA.
  *   - Pointers marked [dev|host] may be device pointers or host pointers (pinned host memory
@@ -150,6 +151,14 @@ int nb_get_stats(nb_ctx *ctx, double out[4], int64_t hist[64]);
  * Fig. 8): split = 0 chooses the number of j-splits automatically (default), split >= 1
  * forces it.  jlanes = 0 automatic, else lanes of a warp that share one i (1, 2, 4 .. 32).  */
 int nb_set_tuning(nb_ctx *ctx, int split, int jlanes);
+
+/* Arithmetic of the evaluation step.  0 (default): IEEE binary64 throughout.  1: the paper's own
+ * mixed scheme (section 5.7): predicted data stay double, the nine differences
+ * r_ij, v_ij, a_ij are formed in double and rounded to float, the pair arithmetic of Eq. 8-10 is
+ * float, pair terms are summed in float within a j-tile (64 or 128 j) and the tile sums in double
+ * (reading G27).  Relative error of a force ~1e-7 of sum_j |pair term| instead of
+ * ~1e-16; everything else (predictor, corrector, time steps, energy) stays binary64.        */
+int nb_set_precision(nb_ctx *ctx, int mode);
 
 /* Driver of nb_run_until / nb_run_steps: 1 (default) = device-driven CUDA-graph batches,
  * 0 = the host issues nb_next_block / nb_predict / nb_force / nb_correct_and_step per step.

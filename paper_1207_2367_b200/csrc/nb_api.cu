@@ -412,6 +412,15 @@ extern "C" int nb_set_tuning(nb_ctx *ctx, int split, int jlanes)
     return NB_OK;
 }
 
+extern "C" int nb_set_precision(nb_ctx *ctx, int mode)
+{
+    if (!ctx) return NB_EINVAL;
+    if (mode != 0 && mode != 1) return set_err(ctx, NB_EINVAL, "nb_set_precision: 0 (FP64) or 1 (mixed SP/DP)");
+    ctx->precision = mode;
+    ctx->evaluated = false;
+    return NB_OK;
+}
+
 extern "C" int nb_set_loop_mode(nb_ctx *ctx, int device_driven)
 {
     if (!ctx) return NB_EINVAL;

@@ -90,6 +90,50 @@ __device__ __forceinline__ void pair_body(const double xi, const double yi, cons
     A.sz = fma(w, tz, A.sz);
 }
 
+// The same pair in the paper's mixed precision (reading G27): the nine
+// differences are formed in double from the double records and rounded to float, everything
+// else of Eq. 8-10 is float arithmetic (FFMA/FMUL on the FP32 pipe, MUFU.RSQ), and the pair
+// terms are summed in float within one j-tile (the caller adds the tile sums in double).
+// FP64-pipe work per pair: 9 DADD + 10 F2F instead of 53 instructions.
+struct AccF {
+    float ax, ay, az, jx, jy, jz, sx, sy, sz;
+};
+template <bool GUARD0>
+__device__ __forceinline__ void pair_body_mx(const double xi, const double yi, const double zi,
+                                             const double vxi, const double vyi, const double vzi,
+                                             const double axi, const double ayi, const double azi,
+                                             const double *__restrict__ q, const float eps2, AccF &A)
+{
+    const double2 p0 = *reinterpret_cast<const double2 *>(q);
+    const double2 p1 = *reinterpret_cast<const double2 *>(q + 2);
+    const double2 p2 = *reinterpret_cast<const double2 *>(q + 4);
+    const double2 p3 = *reinterpret_cast<const double2 *>(q + 6);
+    const double2 p4 = *reinterpret_cast<const double2 *>(q + 8);
+    const float dx = (float)(p0.x - xi), dy = (float)(p0.y - yi), dz = (float)(p1.x - zi);
+    const float dvx = (float)(p1.y - vxi), dvy = (float)(p2.x - vyi), dvz = (float)(p2.y - vzi);
+    const float dax = (float)(p3.x - axi), day = (float)(p3.y - ayi), daz = (float)(p4.x - azi);
+    const float mj = (float)p4.y;
+    const float s = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, eps2)));
+    const float rv = fmaf(dx, dvx, fmaf(dy, dvy, dz * dvz));
+    const float vr = fmaf(dx, dax, fmaf(dy, day, fmaf(dz, daz, fmaf(dvx, dvx, fmaf(dvy, dvy, dvz * dvz)))));
+    float y = rsqrtf(s);
+    if (GUARD0) {  // eps = 0: the self term (s = 0) contributes nothing (G12)
+        if (s == 0.0f) y = 0.0f;
+    }
+    const float P = y * y;             // 1/s
+    const float w = (mj * y) * P;      // m_j s^(-3/2)
+    const float qq = -3.0f * P;
+    const float g = rv * qq;           // -3 alpha
+    const float b3 = fmaf(g * g, -1.0f / 3.0f, qq * vr);  // -3 beta
+    const float g2 = g + g;
+    const float ux = fmaf(g, dx, dvx), uy = fmaf(g, dy, dvy), uz = fmaf(g, dz, dvz);
+    A.ax = fmaf(w, dx, A.ax); A.ay = fmaf(w, dy, A.ay); A.az = fmaf(w, dz, A.az);
+    A.jx = fmaf(w, ux, A.jx); A.jy = fmaf(w, uy, A.jy); A.jz = fmaf(w, uz, A.jz);
+    float tx = fmaf(g2, ux, dax), ty = fmaf(g2, uy, day), tz = fmaf(g2, uz, daz);
+    tx = fmaf(b3, dx, tx); ty = fmaf(b3, dy, ty); tz = fmaf(b3, dz, tz);
+    A.sx = fmaf(w, tx, A.sx); A.sy = fmaf(w, ty, A.sy); A.sz = fmaf(w, tz, A.sz);
+}
+
 // ---- mbarrier / bulk-copy primitives (PTX, sm_90+; SASS: SYNCS.*, UBLKCP) ---------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
@@ -132,7 +176,7 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 // JLT = 1: one i per thread.  JLT = 0: JL (runtime, power of two <= 32) consecutive lanes share
 // one i and stride through the tile.  `tc` counts the tiles this CTA has consumed so far: ring
 // stage = tc & 1, mbarrier phase = (tc >> 1) & 1, so the ring carries over from item to item.
-template <int NT, int TJ, int JLT, bool GUARD0, int UNR>
+template <int NT, int TJ, int JLT, bool GUARD0, bool MX, int UNR>
 __device__ __forceinline__ void force_item(const double *__restrict__ jp, const int32_t *__restrict__ active,
                                            const int m, const int ib, const int sp, const int tiles_total,
                                            const int tiles_per_split, const int JL, const double eps2,
@@ -177,20 +221,37 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
         const unsigned sg = tc & 1u;
         mbar_wait(&full[sg], (tc >> 1) & 1u);
         if (!warp_idle) {
-            Acc9 A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
             const double *q = tile[sg];
-            if (JLT) {
+            if (MX) {
+                AccF A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+                const float eps2f = (float)eps2;
+                if (JLT) {
 #pragma unroll UNR
-                for (int jj = 0; jj < TJ; ++jj)
-                    pair_body<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
-            } else {
+                    for (int jj = 0; jj < TJ; ++jj)
+                        pair_body_mx<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2f, A);
+                } else {
 #pragma unroll 2
-                for (int jj = jl; jj < TJ; jj += JL)
-                    pair_body<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
+                    for (int jj = jl; jj < TJ; jj += JL)
+                        pair_body_mx<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2f, A);
+                }
+                T.ax += (double)A.ax; T.ay += (double)A.ay; T.az += (double)A.az;
+                T.jx += (double)A.jx; T.jy += (double)A.jy; T.jz += (double)A.jz;
+                T.sx += (double)A.sx; T.sy += (double)A.sy; T.sz += (double)A.sz;
+            } else {
+                Acc9 A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+                if (JLT) {
+#pragma unroll UNR
+                    for (int jj = 0; jj < TJ; ++jj)
+                        pair_body<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
+                } else {
+#pragma unroll 2
+                    for (int jj = jl; jj < TJ; jj += JL)
+                        pair_body<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
+                }
+                T.ax += A.ax; T.ay += A.ay; T.az += A.az;
+                T.jx += A.jx; T.jy += A.jy; T.jz += A.jz;
+                T.sx += A.sx; T.sy += A.sy; T.sz += A.sz;
             }
-            T.ax += A.ax; T.ay += A.ay; T.az += A.az;
-            T.jx += A.jx; T.jy += A.jy; T.jz += A.jz;
-            T.sx += A.sx; T.sy += A.sy; T.sz += A.sz;
         }
         __syncthreads();  // every warp is done reading tile[sg]
         if (tid == 0 && it + NS < nt) {
@@ -222,7 +283,7 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
 }
 
 // grid.x: i-blocks, grid.y: j-splits; geometry passed by the host.
-template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int UNR = 4>
+template <int NT, int TJ, int MINB, int JLT, bool GUARD0, bool MX = false, int UNR = 4>
 __global__ void __launch_bounds__(NT, MINB)
     k_force(const double *__restrict__ jp, const int32_t *__restrict__ active, const int m,
             const int tiles_total, const int tiles_per_split, const int JLr, const double eps2,
@@ -237,7 +298,7 @@ __global__ void __launch_bounds__(NT, MINB)
     }
     __syncthreads();
     unsigned tc = 0;
-    force_item<NT, TJ, JLT, GUARD0, UNR>(jp, active, m, blockIdx.x, blockIdx.y, tiles_total, tiles_per_split,
+    force_item<NT, TJ, JLT, GUARD0, MX, UNR>(jp, active, m, blockIdx.x, blockIdx.y, tiles_total, tiles_per_split,
                                          JLT ? 1 : JLr, eps2, out, cstride, sstride, tile, full, tc);
 }
 
@@ -245,7 +306,7 @@ __global__ void __launch_bounds__(NT, MINB)
 // resident CTAs; the set size and the geometry are read from the control block the scheduler
 // kernel of the same step wrote; CTA b takes the work items b, b + gridDim.x, ...  Item w is
 // (i-block w % n_ib, split w / n_ib), so concurrently running CTAs stream the same j-split.
-template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int UNR = 4>
+template <int NT, int TJ, int MINB, int JLT, bool GUARD0, bool MX = false, int UNR = 4>
 __global__ void __launch_bounds__(NT, MINB)
     k_force_persistent(const double *__restrict__ jp, const int32_t *__restrict__ active_list, const int64_t N,
                        const int64_t Npad, const double eps2, double *__restrict__ f1,
@@ -270,7 +331,7 @@ __global__ void __launch_bounds__(NT, MINB)
     const long long items = (long long)g.n_ib * g.S;
     unsigned tc = 0;
     for (long long w = blockIdx.x; w < items; w += gridDim.x)
-        force_item<NT, TJ, JLT, GUARD0, UNR>(jp, active, m, (int)(w % g.n_ib), (int)(w / g.n_ib), tiles_total,
+        force_item<NT, TJ, JLT, GUARD0, MX, UNR>(jp, active, m, (int)(w % g.n_ib), (int)(w / g.n_ib), tiles_total,
                                              g.tps, g.JL, eps2, out, cstride, sstride, tile, full, tc);
 }
 
@@ -398,12 +459,15 @@ template <int NT, int TJ, int MINB, int JLT>
 static void launch_variant(nb_ctx *ctx, dim3 grid, const int32_t *active, int m, int tiles_total,
                            int tps, int JL, double *out, size_t cstride, size_t sstride)
 {
-    if (ctx->eps == 0.0)
-        k_force<NT, TJ, MINB, JLT, true><<<grid, NT, 0, ctx->stream>>>(
-            ctx->jp, active, m, tiles_total, tps, JL, ctx->eps2, out, cstride, sstride);
-    else
-        k_force<NT, TJ, MINB, JLT, false><<<grid, NT, 0, ctx->stream>>>(
-            ctx->jp, active, m, tiles_total, tps, JL, ctx->eps2, out, cstride, sstride);
+#define NB_KF(G0, MXP)                                                                 \
+    k_force<NT, TJ, MINB, JLT, G0, MXP><<<grid, NT, 0, ctx->stream>>>(ctx->jp, active, m, tiles_total, tps, JL, \
+                                                                      ctx->eps2, out, cstride, sstride)
+    const bool g0 = ctx->eps == 0.0, mx = ctx->precision == 1;
+    if (g0 && mx) NB_KF(true, true);
+    else if (g0) NB_KF(true, false);
+    else if (mx) NB_KF(false, true);
+    else NB_KF(false, false);
+#undef NB_KF
 }
 
 int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m)
@@ -449,17 +513,19 @@ int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m)
 int enqueue_force_persistent(nb_ctx *ctx)
 {
     const unsigned gA = (unsigned)(ctx->n_sm * ctx->occ[2]), gB = (unsigned)(ctx->n_sm * ctx->occ[3]);
-    if (ctx->eps == 0.0) {
-        k_force_persistent<NT_A, TJ_A, MINB_A, 1, true><<<gA, NT_A, 0, ctx->stream>>>(
-            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);
-        k_force_persistent<NT_B, TJ_B, MINB_B, 0, true><<<gB, NT_B, 0, ctx->stream>>>(
-            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);
-    } else {
-        k_force_persistent<NT_A, TJ_A, MINB_A, 1, false><<<gA, NT_A, 0, ctx->stream>>>(
-            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);
-        k_force_persistent<NT_B, TJ_B, MINB_B, 0, false><<<gB, NT_B, 0, ctx->stream>>>(
-            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);
-    }
+#define NB_KP(G0, MXP)                                                                                      \
+    do {                                                                                                    \
+        k_force_persistent<NT_A, TJ_A, MINB_A, 1, G0, MXP><<<gA, NT_A, 0, ctx->stream>>>(                     \
+            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);           \
+        k_force_persistent<NT_B, TJ_B, MINB_B, 0, G0, MXP><<<gB, NT_B, 0, ctx->stream>>>(                     \
+            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);           \
+    } while (0)
+    const bool g0 = ctx->eps == 0.0, mx = ctx->precision == 1;
+    if (g0 && mx) NB_KP(true, true);
+    else if (g0) NB_KP(true, false);
+    else if (mx) NB_KP(false, true);
+    else NB_KP(false, false);
+#undef NB_KP
     NB_LAUNCH_CHECK(ctx, "k_force_persistent");
     k_reduce_persistent<<<(unsigned)(2 * ctx->n_sm), 256, 0, ctx->stream>>>(ctx->partials, ctx->ctl, ctx->f1, (size_t)ctx->Npad);
     NB_LAUNCH_CHECK(ctx, "k_reduce_persistent");

@@ -54,6 +54,7 @@ static int build_graph(nb_ctx *ctx)
     if (e3 != cudaSuccess) return set_err(ctx, NB_ECUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e3));
     ctx->graph_batch = B;
     ctx->graph_split = ctx->force_split; ctx->graph_jlanes = ctx->force_jlanes;
+    ctx->graph_precision = ctx->precision;
     return NB_OK;
 }
 
@@ -67,7 +68,8 @@ void graph_release(nb_ctx *ctx)
 int graph_run(nb_ctx *ctx, double t_end, int64_t max_steps, int64_t *n_steps)
 {
     // tuning knobs are kernel arguments of the captured nodes: re-capture when they changed
-    if (ctx->step_graph && (ctx->graph_split != ctx->force_split || ctx->graph_jlanes != ctx->force_jlanes))
+    if (ctx->step_graph && (ctx->graph_split != ctx->force_split || ctx->graph_jlanes != ctx->force_jlanes ||
+                            ctx->graph_precision != ctx->precision))
         graph_release(ctx);
     {
         const int rc = reserve_partials(ctx, ctx->partials_limit);  // no allocation inside a replay

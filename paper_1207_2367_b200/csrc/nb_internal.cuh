@@ -177,12 +177,13 @@ struct nb_ctx {
     nb::StepCtl *h_ctl;             // pinned host copy, refreshed after every graph launch
     cudaGraphExec_t step_graph;     // `graph_batch` block steps captured once per context
     int graph_batch;
-    int graph_split, graph_jlanes;  // tuning knobs the captured graph was built with
+    int graph_split, graph_jlanes, graph_precision;  // knobs the captured graph was built with
     int64_t launches_per_batch;     // kernels in one replay of step_graph
     int use_graph;                  // 1: nb_run_until / nb_run_steps drive the loop from the device
 
     // tuning
     int force_split, force_jlanes;
+    int precision;                  // 0: FP64 throughout (default); 1: the paper's mixed SP/DP pair arithmetic
     int64_t last_launch[5];
     int occ[8];                     // resident CTAs per SM of each evaluation-kernel variant
 

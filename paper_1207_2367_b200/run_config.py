@@ -21,6 +21,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 FLOPS = 85.0
+PRECISION = 0   # nb_set_precision mode of this run (--precision)
 PEAK = 148 * 64 * 2 * 1.965e9
 
 
@@ -47,6 +48,7 @@ def run_integration(nb, cfg, c, N, t_end, n_steps, loop=None):
     g = nb.NBody(_dev(pos), _dev(vel), _dev(m), c["eps"], c["eta"], dt_min=c["dt_min"], dt_max=c["dt_max"])
     if loop is not None:
         nb.nb_set_loop_mode(g.ctx, loop)
+    nb.nb_set_precision(g.ctx, PRECISION)
     t0 = time.perf_counter(); g.startup(); g.sync(); t_start = time.perf_counter() - t0
     e0 = g.energy()
     out = {"config": cfg, "name": c["name"], "N": N, "eps": c["eps"], "eta": c["eta"],
@@ -80,6 +82,7 @@ def run_force(nb, cfg, c, Ns, ms_list):
         pos, vel, m, accp = config_inputs(cfg, N)
         g = nb.NBody(_dev(pos), _dev(vel), _dev(m), c["eps"], 0.45)
         nb.nb_set_pred_acc(g.ctx, _dev(accp))
+        nb.nb_set_precision(g.ctx, PRECISION)
         for mm in (ms_list or [N]):
             idx = None if mm == N else _dev(active_subset(N, mm, c.get("subset_seed", 40)), torch.int32)
             reps = 0 if mm * N > 4e12 else (1 if mm * N > 5e11 else 3)
@@ -154,6 +157,7 @@ def run_fig1(nb, Ns, etas, t_end=4.5, every=0.5, eps=1e-4):
         pos, vel, m = plummer(N, seed=1500 + int(np.log2(N)))
         for eta in etas:
             g = nb.NBody(_dev(pos), _dev(vel), _dev(m), eps, eta, dt_min=2.0 ** -25, dt_max=2.0 ** -4)
+            nb.nb_set_precision(g.ctx, PRECISION)
             g.startup(); g.sync()
             e0 = g.energy(); L0 = np.linalg.norm(e0[6:9])
             dE, dL = [], []
@@ -171,7 +175,7 @@ def run_fig1(nb, Ns, etas, t_end=4.5, every=0.5, eps=1e-4):
                          "pairs": st["n_pairs"] - 2.0 * N * N, "wall_s": wall})
             print(json.dumps(rows[-1]), file=sys.stderr, flush=True)
             g.close()
-    return {"experiment": "fig1_energy_vs_eta", "eps": eps, "t_end": t_end, "sample_every": every, "rows": rows}
+    return {"experiment": "fig1_energy_vs_eta", "precision": "mixed" if PRECISION else "fp64", "eps": eps, "t_end": t_end, "sample_every": every, "rows": rows}
 
 
 def run_probe(nb):
@@ -209,9 +213,13 @@ def main():
     ap.add_argument("--ns", default=None, help="comma-separated N list for --experiment fig1")
     ap.add_argument("--heavy-frac", type=float, default=0.05)
     ap.add_argument("--loop", type=int, default=None, choices=[0, 1], help="0: host-driven loop, 1: device-driven (default)")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"],
+                    help="evaluation arithmetic: fp64 (default) or the paper's mixed SP/DP scheme (PAPER.md:287)")
     a = ap.parse_args()
     import paper_1207_2367_b200 as nb
     from workloads import CONFIGS
+    global PRECISION
+    PRECISION = 1 if a.precision == "mixed" else 0
     if a.experiment == "splitj":
         N = a.n or (1 << 20)
         ms = [1, 2, 4, 8, 16, 32, 64, 128, 256, 1024, 4096, 16384, 65536, 262144]
@@ -240,6 +248,7 @@ def main():
     else:
         N = a.n or c["N"]
         out = run_force(nb, 4, c, [N], [mm for mm in c["m"] if mm <= N])
+    out["precision"] = a.precision
     print(json.dumps(out), flush=True)
 
 
