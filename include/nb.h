@@ -71,6 +71,13 @@ int nb_set_limits(nb_ctx *ctx, double dt_min, double dt_max, double eta_init);
  * sqrt(|a|/|snap|))) clamped to the limits.  Two full-N evaluations (2 N^2 pairs).          */
 int nb_startup(nb_ctx *ctx);
 
+/* The two commits of nb_startup as separate calls, for callers that must exchange the evaluated
+ * values between the passes (j-sharding, nb_set_j_range):  nb_predict(ctx, 0) ->
+ * nb_force(NULL, N) -> [exchange] -> nb_startup_commit(ctx, 1)  (a_pred <- a)  ->
+ * nb_force(NULL, N) -> [exchange] -> nb_startup_commit(ctx, 2)  (commit a, jerk, snap; crackle = 0;
+ * initial dt; the context is started).                                                       */
+int nb_startup_commit(nb_ctx *ctx, int pass);
+
 /* Table 1 row 1: t_next = min_i(t_i + dt_i) and the ascending list of the
  * particles with t_i + dt_i == t_next, built on the device.  Returns both [host].           */
 int nb_next_block(nb_ctx *ctx, double *t_next, int64_t *n_active);
@@ -152,6 +159,23 @@ int nb_get_stats(nb_ctx *ctx, double out[4], int64_t hist[64]);
  * forces it.  jlanes = 0 automatic, else lanes of a warp that share one i (1, 2, 4 .. 32).  */
 int nb_set_tuning(nb_ctx *ctx, int split, int jlanes);
 
+/* j-sharding across GPUs (the paper's decomposition; Table 1 row 7): every
+ * process holds the whole (replicated) state, evaluates the active particles against its own
+ * slice [j_begin, j_end) of the predicted particles only, and the partial (acc, jerk, snap) of
+ * all processes are summed before the corrector:
+ *     nb_next_block -> nb_predict -> nb_force(NULL, m, ...) -> nb_get_forces(buf)
+ *     -> all-reduce(sum) of buf over the processes -> nb_set_forces(buf) -> nb_correct_and_step.
+ * j_begin and j_end must be multiples of 128 (j_end may also be N).  Default [0, N).  With a
+ * proper slice set, nb_run_until / nb_run_steps refuse (NB_ESTATE): the exchange is the caller's. */
+int nb_set_j_range(nb_ctx *ctx, int64_t j_begin, int64_t j_end);
+
+/* The (acc, jerk, snap) of the set just evaluated, as one contiguous buffer the caller can
+ * all-reduce: buf [dev|host] [9][n_eval] = {ax, ay, az, jx, jy, jz, sx, sy, sz} x n_eval.
+ * nb_set_forces stores a buffer of that layout back as the evaluated values that
+ * nb_correct_and_step will use.                                                             */
+int nb_get_forces(nb_ctx *ctx, double *buf);
+int nb_set_forces(nb_ctx *ctx, const double *buf);
+
 /* Arithmetic of the evaluation step.  0 (default): IEEE binary64 throughout.  1: the paper's own
  * mixed scheme (section 5.7): predicted data stay double, the nine differences
  * r_ij, v_ij, a_ij are formed in double and rounded to float, the pair arithmetic of Eq. 8-10 is
@@ -182,7 +206,6 @@ int nb_probe_fp64_peak(nb_ctx *ctx, int64_t iters, double *flops, float *ms);
  *   4: three registers, the first shared by ALL DFMAs (reuse-cache hit on every instruction but
  *      the one after each scheduler yield)
  *   5: alternating 3-register DFMA and a DADD that shares one source with it (1 fresh read)
- *   6: alternating 3-register DFMA and a DADD with its own sources (2 fresh reads)
  * *cycles_per_inst [host] = SM-clock cycles per warp instruction per SM sub-partition, at the
  * clock `sm_mhz` the caller passes (e.g. the nvidia-smi reading).                          */
 int nb_probe_fp64_operands(nb_ctx *ctx, int mode, int64_t iters, double sm_mhz, double *cycles_per_inst);

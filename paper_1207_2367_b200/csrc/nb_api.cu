@@ -121,6 +121,7 @@ extern "C" int nb_init(nb_ctx **out, int64_t N, const double *pos, const double 
     if (cudaHostAlloc((void **)&ctx->h_ctl, sizeof(StepCtl), cudaHostAllocDefault) != cudaSuccess) return fail(NB_ENOMEM);
     memset(ctx->h_ctl, 0, sizeof(StepCtl));
     ctx->use_graph = 1;
+    ctx->j_begin = 0; ctx->j_end = N;
     if ((rc = query_force_occupancy(ctx))) return fail(rc);
 
     // stage the caller's arrays on the device ([N][3] | [N][3] | [N]) and build the SoA state
@@ -158,6 +159,20 @@ extern "C" int nb_startup(nb_ctx *ctx)
     NB_TRY(launch_startup_commit(ctx, 2));           // commit, crackle = 0, initial dt
     ctx->started = true; ctx->pred_valid = true; ctx->t_pred = 0.0; ctx->t_now = 0.0;
     ctx->have_block = false; ctx->evaluated = false;
+    return NB_OK;
+}
+
+extern "C" int nb_startup_commit(nb_ctx *ctx, int pass)
+{
+    if (!ctx) return NB_EINVAL;
+    if (ctx->started) return set_err(ctx, NB_ESTATE, "nb_startup_commit: already started");
+    if (pass != 1 && pass != 2) return set_err(ctx, NB_EINVAL, "nb_startup_commit: pass is 1 or 2");
+    if (ctx->n_eval != ctx->N) return set_err(ctx, NB_ESTATE, "nb_startup_commit: evaluate all N particles first (nb_force(NULL, N))");
+    NB_TRY(launch_startup_commit(ctx, pass));
+    if (pass == 2) {
+        ctx->started = true; ctx->pred_valid = true; ctx->t_pred = 0.0; ctx->t_now = 0.0;
+        ctx->have_block = false; ctx->evaluated = false;
+    }
     return NB_OK;
 }
 
@@ -256,6 +271,8 @@ extern "C" int nb_run_until(nb_ctx *ctx, double t_end, int64_t *n_steps)
     if (!ctx) return NB_EINVAL;
     if (!isfinite(t_end)) return set_err(ctx, NB_EINVAL, "nb_run_until: bad t_end");
     if (!ctx->started) NB_TRY(nb_startup(ctx));
+    if (ctx->j_begin != 0 || ctx->j_end != ctx->N)
+        return set_err(ctx, NB_ESTATE, "nb_run_until: a j-shard is set (nb_set_j_range); drive the steps call by call and all-reduce nb_get_forces");
     if (ctx->use_graph) return graph_run(ctx, t_end, INT64_MAX, n_steps);
     int64_t n = 0;
     for (;;) {
@@ -273,6 +290,8 @@ extern "C" int nb_run_steps(nb_ctx *ctx, int64_t n, double *log_t, int64_t *log_
 {
     if (!ctx || n < 0) return NB_EINVAL;
     if (!ctx->started) NB_TRY(nb_startup(ctx));
+    if (ctx->j_begin != 0 || ctx->j_end != ctx->N)
+        return set_err(ctx, NB_ESTATE, "nb_run_steps: a j-shard is set (nb_set_j_range)");
     if (ctx->use_graph && !log_t && !log_m && !log_ms) {
         if (n == 0) return NB_OK;
         return graph_run(ctx, __longlong_as_double_host(0x7fefffffffffffffLL), n, nullptr);
@@ -412,6 +431,33 @@ extern "C" int nb_set_tuning(nb_ctx *ctx, int split, int jlanes)
     return NB_OK;
 }
 
+extern "C" int nb_set_j_range(nb_ctx *ctx, int64_t j_begin, int64_t j_end)
+{
+    if (!ctx) return NB_EINVAL;
+    if (j_begin < 0 || j_end > ctx->N || j_begin >= j_end || (j_begin % TILE_ALIGN) != 0 ||
+        (j_end != ctx->N && (j_end % TILE_ALIGN) != 0))
+        return set_err(ctx, NB_EINVAL, "nb_set_j_range: need 0 <= j_begin < j_end <= N, both multiples of %d (j_end may be N)", TILE_ALIGN);
+    ctx->j_begin = j_begin; ctx->j_end = j_end;
+    ctx->evaluated = false;
+    return NB_OK;
+}
+
+extern "C" int nb_get_forces(nb_ctx *ctx, double *buf)
+{
+    if (!ctx || !buf) return NB_EINVAL;
+    if (ctx->n_eval <= 0) return set_err(ctx, NB_ESTATE, "nb_get_forces: nothing evaluated");
+    NB_TRY(launch_f1_contig(ctx, ctx->n_eval, ctx->stage, false));
+    return copy_out(ctx, buf, ctx->stage, 9 * (size_t)ctx->n_eval * sizeof(double));
+}
+
+extern "C" int nb_set_forces(nb_ctx *ctx, const double *buf)
+{
+    if (!ctx || !buf) return NB_EINVAL;
+    if (ctx->n_eval <= 0) return set_err(ctx, NB_ESTATE, "nb_set_forces: nothing evaluated");
+    NB_TRY(copy_in(ctx, ctx->stage, buf, 9 * (size_t)ctx->n_eval * sizeof(double)));
+    return launch_f1_contig(ctx, ctx->n_eval, ctx->stage, true);
+}
+
 extern "C" int nb_set_precision(nb_ctx *ctx, int mode)
 {
     if (!ctx) return NB_EINVAL;
@@ -444,6 +490,6 @@ extern "C" int nb_probe_fp64_peak(nb_ctx *ctx, int64_t iters, double *flops, flo
 
 extern "C" int nb_probe_fp64_operands(nb_ctx *ctx, int mode, int64_t iters, double sm_mhz, double *cycles_per_inst)
 {
-    if (!ctx || iters < 1 || mode < 0 || mode > 6 || !(sm_mhz > 0.0)) return NB_EINVAL;
+    if (!ctx || iters < 1 || mode < 0 || mode > 5 || !(sm_mhz > 0.0)) return NB_EINVAL;
     return launch_probe_operands(ctx, mode, iters, sm_mhz, cycles_per_inst);
 }

@@ -187,10 +187,6 @@ __global__ void __launch_bounds__(512) k_probe_operands(const long long iters, c
                     if (k % 2 == 0) asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(x[k]) : "d"(a[k]), "d"(b[k]));
                     else asm volatile("add.f64 %0, %1, %0;" : "+d"(x[k]) : "d"(a[k - 1]));
                 }
-                if (MODE == 6) {  // 3-register DFMA, then a DADD with its own second operand (2 fresh reads)
-                    if (k % 2 == 0) asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(x[k]) : "d"(a[k]), "d"(b[k]));
-                    else asm volatile("add.f64 %0, %1, %0;" : "+d"(x[k]) : "d"(b[k]));
-                }
             }
         }
     }
@@ -215,8 +211,7 @@ int launch_probe_operands(nb_ctx *ctx, int mode, int64_t iters, double sm_mhz, d
             case 2: k_probe_operands<2><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
             case 3: k_probe_operands<3><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
             case 4: k_probe_operands<4><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
-            case 5: k_probe_operands<5><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
-            default: k_probe_operands<6><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
+            default: k_probe_operands<5><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
         }
         NB_LAUNCH_CHECK(ctx, "k_probe_operands");
     }

@@ -177,8 +177,8 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 // one i and stride through the tile.  `tc` counts the tiles this CTA has consumed so far: ring
 // stage = tc & 1, mbarrier phase = (tc >> 1) & 1, so the ring carries over from item to item.
 template <int NT, int TJ, int JLT, bool GUARD0, bool MX, int UNR>
-__device__ __forceinline__ void force_item(const double *__restrict__ jp, const int32_t *__restrict__ active,
-                                           const int m, const int ib, const int sp, const int tiles_total,
+__device__ __forceinline__ void force_item(const double *__restrict__ jp, const double *__restrict__ jstream,
+                                           const int32_t *__restrict__ active, const int m, const int ib, const int sp, const int tiles_total,
                                            const int tiles_per_split, const int JL, const double eps2,
                                            double *__restrict__ out, const size_t cstride, const size_t sstride,
                                            double (*tile)[TJ * REC], uint64_t *full, unsigned &tc)
@@ -191,7 +191,7 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
     const int jl = tid % JL;                // j-lane
     const int t0 = sp * tiles_per_split;
     const int nt = min(tiles_per_split, tiles_total - t0);
-    const char *src = reinterpret_cast<const char *>(jp) + (size_t)t0 * TILE_BYTES;
+    const char *src = reinterpret_cast<const char *>(jstream) + (size_t)t0 * TILE_BYTES;
 
     if (tid == 0) {
         for (int st = 0; st < NS && st < nt; ++st) {
@@ -285,8 +285,8 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
 // grid.x: i-blocks, grid.y: j-splits; geometry passed by the host.
 template <int NT, int TJ, int MINB, int JLT, bool GUARD0, bool MX = false, int UNR = 4>
 __global__ void __launch_bounds__(NT, MINB)
-    k_force(const double *__restrict__ jp, const int32_t *__restrict__ active, const int m,
-            const int tiles_total, const int tiles_per_split, const int JLr, const double eps2,
+    k_force(const double *__restrict__ jp, const double *__restrict__ jstream,
+            const int32_t *__restrict__ active, const int m, const int tiles_total, const int tiles_per_split, const int JLr, const double eps2,
             double *__restrict__ out, const size_t cstride, const size_t sstride)
 {
     __shared__ __align__(128) double tile[2][TJ * REC];
@@ -298,7 +298,7 @@ __global__ void __launch_bounds__(NT, MINB)
     }
     __syncthreads();
     unsigned tc = 0;
-    force_item<NT, TJ, JLT, GUARD0, MX, UNR>(jp, active, m, blockIdx.x, blockIdx.y, tiles_total, tiles_per_split,
+    force_item<NT, TJ, JLT, GUARD0, MX, UNR>(jp, jstream, active, m, blockIdx.x, blockIdx.y, tiles_total, tiles_per_split,
                                          JLT ? 1 : JLr, eps2, out, cstride, sstride, tile, full, tc);
 }
 
@@ -331,7 +331,7 @@ __global__ void __launch_bounds__(NT, MINB)
     const long long items = (long long)g.n_ib * g.S;
     unsigned tc = 0;
     for (long long w = blockIdx.x; w < items; w += gridDim.x)
-        force_item<NT, TJ, JLT, GUARD0, MX, UNR>(jp, active, m, (int)(w % g.n_ib), (int)(w / g.n_ib), tiles_total,
+        force_item<NT, TJ, JLT, GUARD0, MX, UNR>(jp, jp, active, m, (int)(w % g.n_ib), (int)(w / g.n_ib), tiles_total,
                                              g.tps, g.JL, eps2, out, cstride, sstride, tile, full, tc);
 }
 
@@ -459,8 +459,9 @@ template <int NT, int TJ, int MINB, int JLT>
 static void launch_variant(nb_ctx *ctx, dim3 grid, const int32_t *active, int m, int tiles_total,
                            int tps, int JL, double *out, size_t cstride, size_t sstride)
 {
+    const double *jstream = ctx->jp + (size_t)ctx->j_begin * REC;   // j-shard (nb_set_j_range), else the whole stream
 #define NB_KF(G0, MXP)                                                                 \
-    k_force<NT, TJ, MINB, JLT, G0, MXP><<<grid, NT, 0, ctx->stream>>>(ctx->jp, active, m, tiles_total, tps, JL, \
+    k_force<NT, TJ, MINB, JLT, G0, MXP><<<grid, NT, 0, ctx->stream>>>(ctx->jp, jstream, active, m, tiles_total, tps, JL, \
                                                                       ctx->eps2, out, cstride, sstride)
     const bool g0 = ctx->eps == 0.0, mx = ctx->precision == 1;
     if (g0 && mx) NB_KF(true, true);
@@ -473,11 +474,13 @@ static void launch_variant(nb_ctx *ctx, dim3 grid, const int32_t *active, int m,
 int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m)
 {
     if (m <= 0) return NB_OK;
-    const ForceGeom g = choose_geom(m, ctx->Npad, ctx->n_sm, ctx->occ[0], ctx->occ[1], (int64_t)ctx->partials_limit,
+    // records of the j-shard, padded to whole tiles (records N..Npad-1 have zero mass)
+    const int64_t jlen = (ctx->j_end == ctx->N ? ctx->Npad : ctx->j_end) - ctx->j_begin;
+    const ForceGeom g = choose_geom(m, jlen, ctx->n_sm, ctx->occ[0], ctx->occ[1], (int64_t)ctx->partials_limit,
                                     ctx->force_split, ctx->force_jlanes);
     const bool varA = g.variant == 0;
     const int TJ = varA ? TJ_A : TJ_B;
-    const int64_t tiles = ctx->Npad / TJ;
+    const int64_t tiles = jlen / TJ;
     double *out = ctx->f1;
     size_t cstride = (size_t)ctx->Npad, sstride = 0;
     if (g.S > 1) {
@@ -503,7 +506,7 @@ int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m)
     }
     ctx->last_launch[0] = varA ? NT_A : NT_B; ctx->last_launch[1] = g.JL; ctx->last_launch[2] = g.S;
     ctx->last_launch[3] = (int64_t)g.n_ib * g.S; ctx->last_launch[4] = TJ;
-    ctx->n_pairs += (double)m * (double)ctx->N;
+    ctx->n_pairs += (double)m * (double)(ctx->j_end - ctx->j_begin);
     return NB_OK;
 }
 
@@ -529,6 +532,26 @@ int enqueue_force_persistent(nb_ctx *ctx)
     NB_LAUNCH_CHECK(ctx, "k_force_persistent");
     k_reduce_persistent<<<(unsigned)(2 * ctx->n_sm), 256, 0, ctx->stream>>>(ctx->partials, ctx->ctl, ctx->f1, (size_t)ctx->Npad);
     NB_LAUNCH_CHECK(ctx, "k_reduce_persistent");
+    return NB_OK;
+}
+
+// f1 planes (stride Npad) <-> contiguous [9][m] (the buffer a j-sharded caller all-reduces)
+__global__ void k_f1_contig(double *__restrict__ f1, const size_t f1stride, const int m, double *__restrict__ buf,
+                            const bool to_f1)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int c = blockIdx.y;
+    if (k >= m) return;
+    if (to_f1) f1[c * f1stride + k] = buf[(size_t)c * m + k];
+    else buf[(size_t)c * m + k] = f1[c * f1stride + k];
+}
+
+int launch_f1_contig(nb_ctx *ctx, int64_t m, double *buf, bool to_f1)
+{
+    if (m <= 0) return NB_OK;
+    dim3 g((unsigned)((m + 255) / 256), 9, 1);
+    k_f1_contig<<<g, 256, 0, ctx->stream>>>(ctx->f1, (size_t)ctx->Npad, (int)m, buf, to_f1);
+    NB_LAUNCH_CHECK(ctx, "k_f1_contig");
     return NB_OK;
 }
 

@@ -183,6 +183,7 @@ struct nb_ctx {
 
     // tuning
     int force_split, force_jlanes;
+    int64_t j_begin, j_end;         // j-shard evaluated by nb_force (nb_set_j_range); default [0, N)
     int precision;                  // 0: FP64 throughout (default); 1: the paper's mixed SP/DP pair arithmetic
     int64_t last_launch[5];
     int occ[8];                     // resident CTAs per SM of each evaluation-kernel variant
@@ -207,6 +208,7 @@ int query_force_occupancy(nb_ctx *ctx);
 int enqueue_force_persistent(nb_ctx *ctx);   // both variants + reduction, geometry read from ctx->ctl
 // f1[c][k] -> out[q][k][3] (q = 0 acc, 1 jerk, 2 snap) contiguous in ctx->stage
 int launch_unpack_f1(nb_ctx *ctx, int64_t m);
+int launch_f1_contig(nb_ctx *ctx, int64_t m, double *buf, bool to_f1);
 int reserve_partials(nb_ctx *ctx, size_t doubles);
 
 // ----- nb_step.cu

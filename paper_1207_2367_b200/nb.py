@@ -17,10 +17,10 @@ from . import _build
 
 __all__ = [
     "NBError", "lib", "lib_path", "exported_symbols", "NBody",
-    "nb_init", "nb_free", "nb_set_limits", "nb_startup", "nb_next_block", "nb_get_active", "nb_predict",
+    "nb_init", "nb_free", "nb_set_limits", "nb_startup", "nb_startup_commit", "nb_next_block", "nb_get_active", "nb_predict",
     "nb_force", "nb_correct_and_step", "nb_run_until", "nb_run_steps", "nb_energy", "nb_get_state",
     "nb_get_derivs", "nb_get_pred", "nb_set_pred_acc", "nb_set_pred", "nb_get_full_state",
-    "nb_set_full_state", "nb_get_stats", "nb_set_tuning", "nb_set_loop_mode", "nb_set_precision", "nb_get_launch", "nb_probe_fp64_peak",
+    "nb_set_full_state", "nb_get_stats", "nb_set_tuning", "nb_set_loop_mode", "nb_set_precision", "nb_set_j_range", "nb_get_forces", "nb_set_forces", "nb_get_launch", "nb_probe_fp64_peak",
     "nb_probe_fp64_operands", "nb_version", "nb_last_error",
 ]
 
@@ -41,6 +41,7 @@ _SIGS = {
     "nb_init": (C.c_int, [C.POINTER(_vp), _i64, _vp, _vp, _vp, _dbl, _dbl, _vp]),
     "nb_set_limits": (C.c_int, [_vp, _dbl, _dbl, _dbl]),
     "nb_startup": (C.c_int, [_vp]),
+    "nb_startup_commit": (C.c_int, [_vp, C.c_int]),
     "nb_next_block": (C.c_int, [_vp, C.POINTER(_dbl), C.POINTER(_i64)]),
     "nb_get_active": (C.c_int, [_vp, _vp]),
     "nb_predict": (C.c_int, [_vp, _dbl]),
@@ -60,6 +61,9 @@ _SIGS = {
     "nb_set_tuning": (C.c_int, [_vp, C.c_int, C.c_int]),
     "nb_set_loop_mode": (C.c_int, [_vp, C.c_int]),
     "nb_set_precision": (C.c_int, [_vp, C.c_int]),
+    "nb_set_j_range": (C.c_int, [_vp, _i64, _i64]),
+    "nb_get_forces": (C.c_int, [_vp, _vp]),
+    "nb_set_forces": (C.c_int, [_vp, _vp]),
     "nb_get_launch": (C.c_int, [_vp, C.POINTER(_i64)]),
     "nb_probe_fp64_peak": (C.c_int, [_vp, _i64, C.POINTER(_dbl), C.POINTER(C.c_float)]),
     "nb_probe_fp64_operands": (C.c_int, [_vp, C.c_int, _i64, _dbl, C.POINTER(_dbl)]),
@@ -168,6 +172,10 @@ def nb_startup(ctx):
     _check(ctx, lib().nb_startup(ctx))
 
 
+def nb_startup_commit(ctx, npass):
+    _check(ctx, lib().nb_startup_commit(ctx, int(npass)))
+
+
 def nb_next_block(ctx):
     t, m = _dbl(), _i64()
     _check(ctx, lib().nb_next_block(ctx, C.byref(t), C.byref(m)))
@@ -263,6 +271,19 @@ def nb_set_loop_mode(ctx, device_driven=1):
 
 def nb_set_precision(ctx, mode=0):
     _check(ctx, lib().nb_set_precision(ctx, int(mode)))
+
+
+def nb_set_j_range(ctx, j_begin, j_end):
+    _check(ctx, lib().nb_set_j_range(ctx, int(j_begin), int(j_end)))
+
+
+def nb_get_forces(ctx, buf):
+    _check(ctx, lib().nb_get_forces(ctx, _ptr(buf)))
+    return buf
+
+
+def nb_set_forces(ctx, buf):
+    _check(ctx, lib().nb_set_forces(ctx, _ptr(buf)))
 
 
 def nb_get_launch(ctx):

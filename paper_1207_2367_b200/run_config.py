@@ -191,10 +191,9 @@ def run_probe(nb):
     f, ms = nb.nb_probe_fp64_peak(g.ctx, 1 << 17)
     names = {0: "1 register + immediates", 1: "3 distinct registers", 2: "3 registers, one shared by 3 consecutive DFMAs",
              3: "2 distinct registers (a*a+c)", 4: "3 registers, one shared by all DFMAs",
-             5: "3-register DFMA alternating with a DADD sharing one source (per FP64 instruction)",
-             6: "3-register DFMA alternating with an independent DADD (per FP64 instruction)"}
+             5: "3-register DFMA alternating with a DADD sharing one source (per FP64 instruction)"}
     out = {"sm_mhz_assumed": mhz, "dfma_peak_tflops": f / 1e12, "nominal_tflops": PEAK / 1e12,
-           "cycles_per_warp_inst_per_smsp": {names[k]: nb.nb_probe_fp64_operands(g.ctx, k, 20000, mhz) for k in range(7)}}
+           "cycles_per_warp_inst_per_smsp": {names[k]: nb.nb_probe_fp64_operands(g.ctx, k, 20000, mhz) for k in range(6)}}
     g.close()
     return out
 
