@@ -195,3 +195,22 @@ def test_config4_full_size_subsets(nb, oracle, m_act):
     errs = (g17_err(a[sel], ra), g17_err(j[sel], rj), g17_err(s[sel], rs))
     assert max(errs) <= FORCE_TOL, (errs, launch)
     assert launch["ctas"] >= 148
+
+
+@pytest.mark.parametrize("cfg,N,eps", [(3, 1 << 22, 1e-3), (5, 1 << 23, 1e-4)])
+def test_largest_sizes_sampled_rows(nb, oracle, cfg, N, eps):
+    # the largest N of BASELINE.json: top of the config 3 sweep (2^22) and config 5 (2^23, 8.4M particles).
+    # 256 sampled active rows (innermost, outermost, ...) against ALL N predicted particles: the evaluation
+    # runs split-j with thousands of CTAs over the whole 336 / 671 MB stream; the oracle needs ~10 s.
+    if cfg == 3:
+        pos, vel, m, accp = config_inputs(3, N)
+    else:
+        pos, vel, m, _ = config_inputs(5, N)
+        from workloads import mean_field_acc
+        accp = mean_field_acc(pos)
+    rows = _sample_rows(N, m, pos)
+    (a, j, s), launch = gpu_force(nb, pos, vel, accp, m, eps, rows)
+    assert launch["splits"] > 1 and launch["ctas"] >= 148
+    ra, rj, rs = oracle.force(pos, vel, accp, m, eps, rows)
+    errs = (g17_err(a, ra), g17_err(j, rj), g17_err(s, rs))
+    assert max(errs) <= FORCE_TOL, (errs, launch)

@@ -194,3 +194,51 @@ def test_shared_step_conserves_momentum(nb):
     P = g.energy()[3:6]
     assert np.all(np.abs(P) < 5e-15)
     g.close()
+
+
+def test_config2_full_size_lockstep_with_oracle(nb, oracle):
+    """BASELINE.json config 2 at its full size (N = 65 536, eps = 1e-4, eta = 0.45): start-up and the first
+    block steps in lockstep with the oracle's Hermite loop -- same t_next, same active set, same new dt,
+    positions to rounding.  (The whole run to t = 1 is 1.4e12 pairs: hours for the oracle; its
+    conservation properties are checked in test_config2_short_run_properties.)"""
+    c = CONFIGS[2]
+    pos, vel, m, _ = config_inputs(2)
+    g = _mk(nb, pos, vel, m, c["eps"], c["eta"], c["dt_min"], c["dt_max"])
+    g.startup()
+    it = oracle.Integrator(pos, vel, m, eps=c["eps"], eta=c["eta"], dt_min=c["dt_min"], dt_max=c["dt_max"])
+    assert np.array_equal(host(g.state()[3]), it.dt)                  # initial steps: identical decisions
+    for _ in range(40):
+        tn, n = g.next_block()
+        otn, oact = it.next_block()
+        assert tn == otn and n == oact.size
+        assert np.array_equal(host(g.active(n)), oact)
+        g.predict(tn); nb.nb_force(g.ctx, None, n); g.correct_and_step()
+        it.step()
+    r, v, t, dt = [host(x) for x in g.state()]
+    assert np.array_equal(t, it.t) and np.array_equal(dt, it.dt)
+    assert _rel_pos_err(r, it.pos) < 1e-12
+    g.close()
+
+
+def test_config2_short_run_properties(nb):
+    """Config 2 at full size through the device-driven loop for 1/32 time unit: the invariants that hold at
+    any size -- every dt a power of two within the limits, t_i a multiple of dt_i, everybody synchronised at
+    t_end (a multiple of dt_max), energy conserved to truncation level."""
+    c = CONFIGS[2]
+    pos, vel, m, _ = config_inputs(2)
+    g = _mk(nb, pos, vel, m, c["eps"], c["eta"], c["dt_min"], c["dt_max"])
+    g.startup()
+    e0 = g.energy()
+    t_end = c["dt_max"]                                                # 1/16
+    n = g.run_until(t_end)
+    e1 = g.energy()
+    _, _, t, dt = [host(x) for x in g.state()]
+    assert n > 500
+    assert np.all(t == t_end)                                          # synchronised
+    fr, ex = np.frexp(dt)
+    assert np.all(fr == 0.5) and dt.min() >= c["dt_min"] and dt.max() <= c["dt_max"]
+    assert np.all((t / dt) == np.rint(t / dt))
+    assert abs((e1[0] - e0[0]) / e0[0]) < 1e-9
+    st = g.stats()
+    assert st["n_steps"] == n and st["hist"].sum() == n
+    g.close()
