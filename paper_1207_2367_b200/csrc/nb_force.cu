@@ -303,8 +303,8 @@ __global__ void __launch_bounds__(NT, MINB)
 }
 
 // Persistent form for the device-driven block-step loop (nb_graph.cu): a fixed grid of
-// resident CTAs; the set size and the geometry are read from the control block the scheduler
-// kernel of the same step wrote; CTA b takes the work items b, b + gridDim.x, ...  Item w is
+// resident CTAs; the set size and the geometry are read from the control block, where the gather
+// kernel of the same step left them; CTA b takes the work items b, b + gridDim.x, ...  Item w is
 // (i-block w % n_ib, split w / n_ib), so concurrently running CTAs stream the same j-split.
 template <int NT, int TJ, int MINB, int JLT, bool GUARD0, bool MX = false, int UNR = 4>
 __global__ void __launch_bounds__(NT, MINB)
@@ -332,7 +332,7 @@ __global__ void __launch_bounds__(NT, MINB)
     unsigned tc = 0;
     for (long long w = blockIdx.x; w < items; w += gridDim.x)
         force_item<NT, TJ, JLT, GUARD0, MX, UNR>(jp, jp, active, m, (int)(w % g.n_ib), (int)(w / g.n_ib), tiles_total,
-                                             g.tps, g.JL, eps2, out, cstride, sstride, tile, full, tc);
+                                                 g.tps, g.JL, eps2, out, cstride, sstride, tile, full, tc);
 }
 
 // ---- partial-sum reduction (Table 1 row 4): f1[c][k] = sum_s part[s][c][k], s ascending ---
@@ -511,17 +511,18 @@ int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m)
 }
 
 // Device-driven loop: both variants are enqueued with fixed grids (one wave of resident CTAs);
-// the one the scheduler kernel did not select returns at once, as does everything when the
-// control block says `done`.  Then the fixed-grid reduction.
-int enqueue_force_persistent(nb_ctx *ctx)
+// the one the gather kernel did not select returns at once, as does everything when the control
+// block says `done`.
+int enqueue_force_persistent(nb_ctx *ctx, int parity)
 {
+    (void)parity;  // the set size and geometry come from the control block
     const unsigned gA = (unsigned)(ctx->n_sm * ctx->occ[2]), gB = (unsigned)(ctx->n_sm * ctx->occ[3]);
-#define NB_KP(G0, MXP)                                                                                      \
-    do {                                                                                                    \
-        k_force_persistent<NT_A, TJ_A, MINB_A, 1, G0, MXP><<<gA, NT_A, 0, ctx->stream>>>(                     \
-            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);           \
-        k_force_persistent<NT_B, TJ_B, MINB_B, 0, G0, MXP><<<gB, NT_B, 0, ctx->stream>>>(                     \
-            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);           \
+#define NB_KP(G0, MXP)                                                                                       \
+    do {                                                                                                     \
+        k_force_persistent<NT_A, TJ_A, MINB_A, 1, G0, MXP><<<gA, NT_A, 0, ctx->stream>>>(                      \
+            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);            \
+        k_force_persistent<NT_B, TJ_B, MINB_B, 0, G0, MXP><<<gB, NT_B, 0, ctx->stream>>>(                      \
+            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);            \
     } while (0)
     const bool g0 = ctx->eps == 0.0, mx = ctx->precision == 1;
     if (g0 && mx) NB_KP(true, true);
@@ -530,6 +531,7 @@ int enqueue_force_persistent(nb_ctx *ctx)
     else NB_KP(false, false);
 #undef NB_KP
     NB_LAUNCH_CHECK(ctx, "k_force_persistent");
+    ctx->n_launch += 1;  // two kernels
     k_reduce_persistent<<<(unsigned)(2 * ctx->n_sm), 256, 0, ctx->stream>>>(ctx->partials, ctx->ctl, ctx->f1, (size_t)ctx->Npad);
     NB_LAUNCH_CHECK(ctx, "k_reduce_persistent");
     return NB_OK;

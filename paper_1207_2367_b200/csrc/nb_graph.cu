@@ -35,9 +35,9 @@ static int build_graph(nb_ctx *ctx)
     if (e != cudaSuccess) rc = set_err(ctx, NB_ECUDA, "cudaStreamBeginCapture failed: %s", cudaGetErrorString(e));
     const int B = steps_per_batch(ctx);
     for (int b = 0; b < B && rc == NB_OK; ++b) {
-        if ((rc = enqueue_graph_step(ctx)) != NB_OK) break;
-        if ((rc = enqueue_force_persistent(ctx)) != NB_OK) break;
-        rc = enqueue_graph_correct(ctx);
+        if ((rc = enqueue_graph_gather_predict(ctx, b & 1)) != NB_OK) break;
+        if ((rc = enqueue_force_persistent(ctx, b & 1)) != NB_OK) break;
+        rc = enqueue_graph_correct(ctx, b & 1);
     }
     if (e == cudaSuccess) {
         const cudaError_t e2 = cudaStreamEndCapture(cap, &graph);

@@ -39,9 +39,13 @@ struct ForceGeom {
 // Control block of the device-resident block-step loop (nb_graph.cu): lives in device memory,
 // written by the kernels of a step, copied to a pinned mirror once per graph launch.
 struct StepCtl {
-    unsigned long long tmin_bits;  // bits of min_i(t_i + dt_i), accumulated for the NEXT block
-    unsigned int ticket;
+    // Double-buffered by the parity p of the step inside a batch (a kernel argument fixed at capture):
+    // tmin[p] = bits of min_i(t_i + dt_i) of THIS step, complete when the step starts; tmin[1 - p]
+    // collects the minimum for the next step.  cnt[p] = append counter of this step's active list.
+    unsigned long long tmin[2];
+    int cnt[2];
     int done;                      // set when the next block lies beyond t_end / no steps left
+    unsigned int ticket;           // blocks of the gather kernel that have finished (the last one chooses the geometry)
     double t_next, t_end, t_now;
     long long n_active, steps_left, n_steps;
     double n_pairs;
@@ -205,7 +209,7 @@ namespace nb {
 // arithmetic (the body is the same); it only exists for symmetry of the start-up passes.
 int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m);
 int query_force_occupancy(nb_ctx *ctx);
-int enqueue_force_persistent(nb_ctx *ctx);   // both variants + reduction, geometry read from ctx->ctl
+int enqueue_force_persistent(nb_ctx *ctx, int parity);   // both variants; the selected one chooses the geometry
 // f1[c][k] -> out[q][k][3] (q = 0 acc, 1 jerk, 2 snap) contiguous in ctx->stage
 int launch_unpack_f1(nb_ctx *ctx, int64_t m);
 int launch_f1_contig(nb_ctx *ctx, int64_t m, double *buf, bool to_f1);
@@ -223,8 +227,8 @@ int launch_startup_commit(nb_ctx *ctx, int pass);                    // pass 1: 
 int launch_full_state(nb_ctx *ctx, double *state, bool to_ctx);
 int launch_tmax(nb_ctx *ctx);                                        // d_sched->t_next = max t_i
 
-int enqueue_graph_step(nb_ctx *ctx);                                 // count/scan, scatter+predict, correct of one step
-int enqueue_graph_correct(nb_ctx *ctx);
+int enqueue_graph_gather_predict(nb_ctx *ctx, int parity);           // active list + predictor of one step
+int enqueue_graph_correct(nb_ctx *ctx, int parity);           // corrector + bookkeeping
 int launch_graph_begin(nb_ctx *ctx, double t_end, int64_t steps);    // seeds ctl (t_end, steps_left, tmin)
 
 // ----- nb_graph.cu

@@ -529,95 +529,26 @@ int launch_full_state(nb_ctx *ctx, double *state, bool to_ctx)
 // Device-driven block-step loop.  The same steps as above, but every
 // size that depends on the active set is read from the control block StepCtl in device memory,
 // so that the kernels of a step have fixed launch configurations and a batch of steps can be
-// replayed as one CUDA graph without the host learning (t_next, m) in between:
-//   k_g_count            : Table 1 row 1 -- count the due particles per block, scan, publish
-//                          (t_next, m), decide `done`, choose the evaluation geometry
-//   k_g_scatter_predict  : ascending active list + predictor Eq. 3-7 for all N + the part of
-//                          min_i(t_i + dt_i) of the NEXT block that the non-active particles give
-//   (evaluation: k_force_persistent, k_reduce_persistent in nb_force.cu)
-//   k_g_correct          : corrector + new dt for the active set + their part of the next minimum
+// replayed as one CUDA graph without the host learning (t_next, m) in between.  One step is
+//   k_g_gather_predict  : Table 1 row 1 + Eq. 3-7 in ONE pass over the particles: t_next is already
+//                         known (the minimum was collected during the previous step), so a thread
+//                         appends its particle to the active list if it is due (warp-aggregated
+//                         atomic; the order of the list does not affect any result, G18), predicts
+//                         it, and contributes t_i + dt_i of a particle that is NOT due to the minimum
+//                         of the next step
+//                         of the next step; the last block to finish publishes m and the geometry
+//   k_force_persistent  : evaluation (nb_force.cu)
+//   k_reduce_persistent : fixed-order sum of the j-split partials (nb_force.cu)
+//   k_g_correct         : corrector and new dt for the active set, their share of the next minimum,
+//                         bookkeeping
+// All per-step scalars are double-buffered by the parity of the step (StepCtl).
 __global__ void k_g_begin(StepCtl *ctl, const double t_end, const long long steps)
 {
-    ctl->tmin_bits = 0x7ff0000000000000ULL;
-    ctl->ticket = 0; ctl->done = 0;
+    ctl->tmin[0] = 0x7ff0000000000000ULL; ctl->tmin[1] = 0x7ff0000000000000ULL;
+    ctl->cnt[0] = 0; ctl->cnt[1] = 0;
+    ctl->done = 0; ctl->ticket = 0;
     ctl->t_end = t_end; ctl->steps_left = steps; ctl->n_steps = 0; ctl->n_pairs = 0.0;
     for (int b = 0; b < 64; ++b) ctl->hist[b] = 0;
-}
-
-__global__ void __launch_bounds__(SCHED_THREADS)
-    k_g_count(const int64_t N, const int64_t Npad, const double *__restrict__ t, const double *__restrict__ dt,
-              int32_t *__restrict__ blk_count, StepCtl *__restrict__ ctl, const int n_sm, const int occA,
-              const int occB, const int64_t partials_limit, const int force_split, const int force_jlanes)
-{
-    const double tn = __longlong_as_double((long long)ctl->tmin_bits);
-    const int64_t base = (int64_t)blockIdx.x * SCHED_BLOCK + (int64_t)threadIdx.x * SCHED_ITEMS;
-    int cnt = 0;
-#pragma unroll
-    for (int u = 0; u < SCHED_ITEMS; ++u) {
-        const int64_t i = base + u;
-        if (i < N && t[i] + dt[i] == tn) ++cnt;
-    }
-    int total;
-    block_exclusive_scan(cnt, &total);
-    __shared__ bool last;
-    if (threadIdx.x == 0) {
-        blk_count[blockIdx.x] = total;
-        __threadfence();
-        const unsigned int tk = atomicAdd(&ctl->ticket, 1u);
-        last = (tk == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (!last) return;
-    __threadfence();
-    int carry = 0;
-    for (int b0 = 0; b0 < (int)gridDim.x; b0 += SCHED_THREADS) {
-        const int b = b0 + threadIdx.x;
-        const int v = b < (int)gridDim.x ? ((volatile int32_t *)blk_count)[b] : 0;
-        int tot;
-        const int ex = block_exclusive_scan(v, &tot);
-        if (b < (int)gridDim.x) blk_count[b] = carry + ex;
-        carry += tot;
-    }
-    // the last block decides: done?, (t_next, m), and the evaluation geometry.  The split
-    // candidates (choose_split's loop) are scored by one thread each: 65 x a few 64-bit divisions
-    // in a single thread would cost more than the rest of the step.
-    __shared__ ForceGeom sg;
-    __shared__ SplitProblem sp;
-    __shared__ long long scost[MAX_WAVES + 1];
-    __shared__ int ssplit[MAX_WAVES + 1];
-    __shared__ int sdone;
-    const long long m = carry;
-    if (threadIdx.x == 0) {
-        ctl->ticket = 0;
-        sdone = (ctl->steps_left <= 0 || !(tn <= ctl->t_end)) ? 1 : 0;
-        ctl->done = sdone;
-        if (!sdone) sp = geom_begin(sg, m, Npad, n_sm, occA, occB, partials_limit, force_jlanes);
-    }
-    __syncthreads();
-    if (sdone) return;
-    if (threadIdx.x <= MAX_WAVES) {
-        int S;
-        scost[threadIdx.x] = split_candidate(sp, threadIdx.x, &S);
-        ssplit[threadIdx.x] = S;
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        long long best = INT64_MAX;
-        int best_s = 1;
-        for (int w = 0; w <= MAX_WAVES; ++w)
-            if (scost[w] < best) { best = scost[w]; best_s = ssplit[w]; }
-        geom_finish(sg, sp, best_s, force_split);
-        ctl->t_next = tn;
-        ctl->n_active = m;
-        ctl->g = sg;
-        ctl->steps_left -= 1;
-        ctl->n_steps += 1;
-        ctl->n_pairs += (double)m * (double)N;
-        int b = 0;
-        while ((1LL << (b + 1)) <= m) ++b;
-        ctl->hist[b] += 1;
-        ctl->tmin_bits = 0x7ff0000000000000ULL;  // every block has read it: start the next minimum
-    }
 }
 
 __device__ __forceinline__ void block_min_to(double v, unsigned long long *dst)
@@ -635,63 +566,112 @@ __device__ __forceinline__ void block_min_to(double v, unsigned long long *dst)
 }
 
 __global__ void __launch_bounds__(SCHED_THREADS)
-    k_g_scatter_predict(const int64_t N, const int64_t Npad, const int n_sched_blocks, const double *__restrict__ t,
-                        const double *__restrict__ dt, const int32_t *__restrict__ blk_off,
-                        int32_t *__restrict__ active, StepCtl *__restrict__ ctl, const double *__restrict__ mass,
-                        const double *__restrict__ r, const double *__restrict__ v, const double *__restrict__ a,
-                        const double *__restrict__ j, const double *__restrict__ s, const double *__restrict__ c,
-                        double *__restrict__ jp)
+    k_g_gather_predict(const int p, const int64_t N, const int64_t Npad, const double *__restrict__ t,
+                       const double *__restrict__ dt, int32_t *__restrict__ active, StepCtl *__restrict__ ctl,
+                       const double *__restrict__ mass, const double *__restrict__ r, const double *__restrict__ v,
+                       const double *__restrict__ a, const double *__restrict__ j, const double *__restrict__ s,
+                       const double *__restrict__ c, double *__restrict__ jp, const int n_sm, const int occA,
+                       const int occB, const int64_t partials_limit, const int force_split, const int force_jlanes)
 {
-    if (ctl->done) return;
-    const double tn = ctl->t_next;
-    // predictor: one particle per thread (coalesced), grid = ceil(N / 256) blocks
-    {
-        const int64_t i = (int64_t)blockIdx.x * SCHED_THREADS + threadIdx.x;
-        if (i < N) predict_one(i, Npad, tn, t, mass, r, v, a, j, s, c, jp);
+    // every block evaluates the same condition from values no kernel of this step modifies
+    const double tn = __longlong_as_double((long long)ctl->tmin[p]);
+    const bool done = ctl->done || ctl->steps_left <= 0 || !(tn <= ctl->t_end);
+    if (done) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) ctl->done = 1;
+        return;
     }
-    // the first n_sched_blocks blocks also gather the active list of their 2048-particle chunk
-    if (blockIdx.x >= n_sched_blocks) return;
-    const int64_t base = (int64_t)blockIdx.x * SCHED_BLOCK + (int64_t)threadIdx.x * SCHED_ITEMS;
-    bool hit[SCHED_ITEMS];
-    int cnt = 0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) ctl->t_next = tn;
+    const int64_t i = (int64_t)blockIdx.x * SCHED_THREADS + threadIdx.x;
     double vmin = __longlong_as_double(0x7ff0000000000000LL);
-#pragma unroll
-    for (int u = 0; u < SCHED_ITEMS; ++u) {
-        const int64_t i = base + u;
-        hit[u] = false;
-        if (i < N) {
-            const double due = t[i] + dt[i];
-            hit[u] = (due == tn);
-            if (!hit[u]) vmin = fmin(vmin, due);
-        }
-        cnt += hit[u] ? 1 : 0;
+    bool hit = false;
+    if (i < N) {
+        const double due = t[i] + dt[i];
+        hit = (due == tn);
+        if (!hit) vmin = due;
+        predict_one(i, Npad, tn, t, mass, r, v, a, j, s, c, jp);
     }
-    int total;
-    int pos = blk_off[blockIdx.x] + block_exclusive_scan(cnt, &total);
-#pragma unroll
-    for (int u = 0; u < SCHED_ITEMS; ++u)
-        if (hit[u]) active[pos++] = (int32_t)(base + u);
-    block_min_to(vmin, &ctl->tmin_bits);
+    // warp-aggregated append
+    const unsigned mask = __ballot_sync(0xffffffffu, hit);
+    if (mask) {
+        const int lane = threadIdx.x & 31;
+        const int leader = __ffs(mask) - 1;
+        int base = 0;
+        if (lane == leader) base = atomicAdd(&ctl->cnt[p], __popc(mask));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (hit) active[base + __popc(mask & ((1u << lane) - 1u))] = (int32_t)i;
+    }
+    block_min_to(vmin, &ctl->tmin[1 - p]);
+
+    // the last block to finish knows m: it publishes (m, evaluation geometry).  The 65 split
+    // candidates of choose_split are scored by one thread each (a single thread doing the 64-bit
+    // divisions alone costs more than the rest of the step).
+    __shared__ bool last;
+    __shared__ ForceGeom sg;
+    __shared__ SplitProblem sp;
+    __shared__ long long scost[MAX_WAVES + 1];
+    __shared__ int ssplit[MAX_WAVES + 1];
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        last = (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    const int m = *((volatile int *)&ctl->cnt[p]);
+    if (threadIdx.x == 0) {
+        ctl->ticket = 0;
+        sp = geom_begin(sg, m, Npad, n_sm, occA, occB, partials_limit, force_jlanes);
+    }
+    __syncthreads();
+    if (threadIdx.x <= MAX_WAVES) {
+        int S;
+        scost[threadIdx.x] = split_candidate(sp, threadIdx.x, &S);
+        ssplit[threadIdx.x] = S;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        long long best = INT64_MAX;
+        int best_s = 1;
+        for (int w = 0; w <= MAX_WAVES; ++w)
+            if (scost[w] < best) { best = scost[w]; best_s = ssplit[w]; }
+        geom_finish(sg, sp, best_s, force_split);
+        ctl->n_active = m;
+        ctl->g = sg;
+    }
 }
 
+// Corrector and new dt for the active set (grid-stride over its slots), their share of the next
+// minimum, and -- block 0 -- the bookkeeping of the step; that touches only fields which no block of
+// this kernel reads (they read t_next, n_active, g, which the earlier kernels of the step published).
 __global__ void __launch_bounds__(SCHED_THREADS)
-    k_g_correct(const int64_t N, const int64_t Npad, const int32_t *__restrict__ active_list,
-                StepCtl *__restrict__ ctl, const double eta, const double dt_min, const double dt_max,
-                const double *__restrict__ f1, double *__restrict__ ti, double *__restrict__ dti,
-                double *__restrict__ r, double *__restrict__ v, double *__restrict__ a, double *__restrict__ j,
-                double *__restrict__ s, double *__restrict__ c)
+    k_g_correct(const int p, const int64_t N, const int64_t Npad, const int32_t *__restrict__ active_list,
+                       StepCtl *__restrict__ ctl, const double eta, const double dt_min, const double dt_max,
+                       const double *__restrict__ f1, double *__restrict__ ti,
+                       double *__restrict__ dti, double *__restrict__ r, double *__restrict__ v,
+                       double *__restrict__ a, double *__restrict__ j, double *__restrict__ s, double *__restrict__ c)
 {
     if (ctl->done) return;
     const int m = (int)ctl->n_active;
     const double tn = ctl->t_next;
     const int32_t *active = (m == N) ? nullptr : active_list;
     double vmin = __longlong_as_double(0x7ff0000000000000LL);
-    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < m; k += gridDim.x * blockDim.x) {
+    for (int k = blockIdx.x * SCHED_THREADS + threadIdx.x; k < m; k += gridDim.x * SCHED_THREADS) {
         const int64_t i = active ? active[k] : k;
         vmin = fmin(vmin, correct_one(k, i, Npad, tn, eta, dt_min, dt_max, f1, ti, dti, r, v, a, j, s, c));
     }
-    block_min_to(vmin, &ctl->tmin_bits);
-    if (blockIdx.x == 0 && threadIdx.x == 0) ctl->t_now = tn;
+    block_min_to(vmin, &ctl->tmin[1 - p]);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        ctl->t_now = tn;
+        ctl->steps_left -= 1;
+        ctl->n_steps += 1;
+        ctl->n_pairs += (double)m * (double)N;
+        int b = 0;
+        while ((1LL << (b + 1)) <= (long long)m) ++b;
+        ctl->hist[b] += 1;
+        ctl->tmin[p] = 0x7ff0000000000000ULL;   // this step's minimum is consumed: slot p collects the one after next
+        ctl->cnt[p] = 0;
+    }
 }
 
 int launch_graph_begin(nb_ctx *ctx, double t_end, int64_t steps)
@@ -700,34 +680,31 @@ int launch_graph_begin(nb_ctx *ctx, double t_end, int64_t steps)
     NB_LAUNCH_CHECK(ctx, "k_g_begin");
     int g = (int)((ctx->N + SCHED_THREADS - 1) / SCHED_THREADS);
     if (g > 4 * ctx->n_sm) g = 4 * ctx->n_sm;
-    k_tmin<<<g, SCHED_THREADS, 0, ctx->stream>>>(ctx->N, ctx->t, ctx->dt, &ctx->ctl->tmin_bits);
+    k_tmin<<<g, SCHED_THREADS, 0, ctx->stream>>>(ctx->N, ctx->t, ctx->dt, &ctx->ctl->tmin[0]);
     NB_LAUNCH_CHECK(ctx, "k_tmin");
     return NB_OK;
 }
 
-int enqueue_graph_step(nb_ctx *ctx)
+int enqueue_graph_gather_predict(nb_ctx *ctx, int parity)
 {
-    const int nb = (int)ctx->n_sched_blocks;
-    k_g_count<<<nb, SCHED_THREADS, 0, ctx->stream>>>(ctx->N, ctx->Npad, ctx->t, ctx->dt, ctx->blk_count, ctx->ctl,
-                                                      ctx->n_sm, ctx->occ[0], ctx->occ[1],
-                                                      (int64_t)ctx->partials_limit, ctx->force_split,
-                                                      ctx->force_jlanes);
-    NB_LAUNCH_CHECK(ctx, "k_g_count");
     const unsigned np = (unsigned)((ctx->N + SCHED_THREADS - 1) / SCHED_THREADS);
-    k_g_scatter_predict<<<np, SCHED_THREADS, 0, ctx->stream>>>(ctx->N, ctx->Npad, nb, ctx->t, ctx->dt, ctx->blk_count,
-                                                                ctx->active, ctx->ctl, ctx->mass, ctx->r, ctx->v,
-                                                                ctx->a, ctx->j, ctx->s, ctx->c, ctx->jp);
-    NB_LAUNCH_CHECK(ctx, "k_g_scatter_predict");
+    k_g_gather_predict<<<np, SCHED_THREADS, 0, ctx->stream>>>(parity, ctx->N, ctx->Npad, ctx->t, ctx->dt, ctx->active,
+                                                               ctx->ctl, ctx->mass, ctx->r, ctx->v, ctx->a, ctx->j,
+                                                               ctx->s, ctx->c, ctx->jp, ctx->n_sm, ctx->occ[0], ctx->occ[1],
+                                                               (int64_t)ctx->partials_limit, ctx->force_split,
+                                                               ctx->force_jlanes);
+    NB_LAUNCH_CHECK(ctx, "k_g_gather_predict");
     return NB_OK;
 }
 
-int enqueue_graph_correct(nb_ctx *ctx)
+int enqueue_graph_correct(nb_ctx *ctx, int parity)
 {
     int64_t g = (ctx->N + SCHED_THREADS - 1) / SCHED_THREADS;
     if (g > 4 * ctx->n_sm) g = 4 * ctx->n_sm;
-    k_g_correct<<<(unsigned)g, SCHED_THREADS, 0, ctx->stream>>>(ctx->N, ctx->Npad, ctx->active, ctx->ctl, ctx->eta,
-                                                               ctx->dt_min, ctx->dt_max, ctx->f1, ctx->t, ctx->dt,
-                                                               ctx->r, ctx->v, ctx->a, ctx->j, ctx->s, ctx->c);
+    k_g_correct<<<(unsigned)g, SCHED_THREADS, 0, ctx->stream>>>(parity, ctx->N, ctx->Npad, ctx->active, ctx->ctl,
+                                                                      ctx->eta, ctx->dt_min, ctx->dt_max,
+                                                                      ctx->f1, ctx->t, ctx->dt, ctx->r, ctx->v, ctx->a,
+                                                                      ctx->j, ctx->s, ctx->c);
     NB_LAUNCH_CHECK(ctx, "k_g_correct");
     return NB_OK;
 }
