@@ -153,7 +153,7 @@ extern "C" int nb_startup(nb_ctx *ctx)
     if (ctx->started) return set_err(ctx, NB_ESTATE, "nb_startup: already started");
     // predicted stream <- (r, v, a = 0) at t = 0 (all t_i = 0, derivatives 0: the predictor is the identity)
     NB_TRY(launch_predict(ctx, 0.0));
-    NB_TRY(launch_force(ctx, nullptr, ctx->N));      // pass 1: a, jerk (snap lacks the m da term)
+    NB_TRY(launch_force(ctx, nullptr, ctx->N, true)); // pass 1: a, jerk only (its snap would lack the m da term)
     NB_TRY(launch_startup_commit(ctx, 1));           // a_pred <- a
     NB_TRY(launch_force(ctx, nullptr, ctx->N));      // pass 2: a, jerk, snap
     NB_TRY(launch_startup_commit(ctx, 2));           // commit, crackle = 0, initial dt

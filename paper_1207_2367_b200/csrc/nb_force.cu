@@ -38,7 +38,10 @@ __device__ __forceinline__ double rsqrt_seed(double s)
 //   s = |dr|^2 + eps^2, w = m_j s^(-3/2), g = -3 (dr.dv)/s, b3 = -3 beta,
 //   u = dv + g dr,  A0 = w dr,  A1 = w u,  A2 = w (da + 2 g u + b3 dr).
 // q points at the packed record {x y z vx vy vz ax ay az m} of particle j in shared memory.
-template <bool GUARD0>
+// SNAP = false (start-up pass 1, G8: only a and jerk are wanted; the snap of that pass would be
+// discarded): the a_ij differences, r.a, beta and the snap accumulation are left out -- 31 instead
+// of 53 FP64 instructions; a and jerk are computed by the same expressions.
+template <bool GUARD0, bool SNAP = true>
 __device__ __forceinline__ void pair_body(const double xi, const double yi, const double zi,
                                           const double vxi, const double vyi, const double vzi,
                                           const double axi, const double ayi, const double azi,
@@ -81,6 +84,7 @@ __device__ __forceinline__ void pair_body(const double xi, const double yi, cons
     A.jx = fma(w, ux, A.jx);
     A.jy = fma(w, uy, A.jy);
     A.jz = fma(w, uz, A.jz);
+    if (!SNAP) return;  // everything that only feeds the snap above is dead code in this instantiation
     double tx = fma(g2, ux, dax), ty = fma(g2, uy, day), tz = fma(g2, uz, daz);
     tx = fma(b3, dx, tx);
     ty = fma(b3, dy, ty);
@@ -176,7 +180,8 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 // JLT = 1: one i per thread.  JLT = 0: JL (runtime, power of two <= 32) consecutive lanes share
 // one i and stride through the tile.  `tc` counts the tiles this CTA has consumed so far: ring
 // stage = tc & 1, mbarrier phase = (tc >> 1) & 1, so the ring carries over from item to item.
-template <int NT, int TJ, int JLT, bool GUARD0, bool MX, int UNR>
+// MX: 0 = FP64, 1 = mixed precision (reading G27), 2 = FP64 acceleration and jerk only
+template <int NT, int TJ, int JLT, bool GUARD0, int MX, int UNR>
 __device__ __forceinline__ void force_item(const double *__restrict__ jp, const double *__restrict__ jstream,
                                            const int32_t *__restrict__ active, const int m, const int ib, const int sp, const int tiles_total,
                                            const int tiles_per_split, const int JL, const double eps2,
@@ -222,7 +227,7 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
         mbar_wait(&full[sg], (tc >> 1) & 1u);
         if (!warp_idle) {
             const double *q = tile[sg];
-            if (MX) {
+            if (MX == 1) {
                 AccF A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
                 const float eps2f = (float)eps2;
                 if (JLT) {
@@ -242,11 +247,11 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
                 if (JLT) {
 #pragma unroll UNR
                     for (int jj = 0; jj < TJ; ++jj)
-                        pair_body<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
+                        pair_body<GUARD0, MX != 2>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
                 } else {
 #pragma unroll 2
                     for (int jj = jl; jj < TJ; jj += JL)
-                        pair_body<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
+                        pair_body<GUARD0, MX != 2>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
                 }
                 T.ax += A.ax; T.ay += A.ay; T.az += A.az;
                 T.jx += A.jx; T.jy += A.jy; T.jz += A.jz;
@@ -283,7 +288,7 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
 }
 
 // grid.x: i-blocks, grid.y: j-splits; geometry passed by the host.
-template <int NT, int TJ, int MINB, int JLT, bool GUARD0, bool MX = false, int UNR = 4>
+template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int MX = 0, int UNR = 4>
 __global__ void __launch_bounds__(NT, MINB)
     k_force(const double *__restrict__ jp, const double *__restrict__ jstream,
             const int32_t *__restrict__ active, const int m, const int tiles_total, const int tiles_per_split, const int JLr, const double eps2,
@@ -306,7 +311,7 @@ __global__ void __launch_bounds__(NT, MINB)
 // resident CTAs; the set size and the geometry are read from the control block, where the gather
 // kernel of the same step left them; CTA b takes the work items b, b + gridDim.x, ...  Item w is
 // (i-block w % n_ib, split w / n_ib), so concurrently running CTAs stream the same j-split.
-template <int NT, int TJ, int MINB, int JLT, bool GUARD0, bool MX = false, int UNR = 4>
+template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int MX = 0, int UNR = 4>
 __global__ void __launch_bounds__(NT, MINB)
     k_force_persistent(const double *__restrict__ jp, const int32_t *__restrict__ active_list, const int64_t N,
                        const int64_t Npad, const double eps2, double *__restrict__ f1,
@@ -457,21 +462,23 @@ int reserve_partials(nb_ctx *ctx, size_t need)
 
 template <int NT, int TJ, int MINB, int JLT>
 static void launch_variant(nb_ctx *ctx, dim3 grid, const int32_t *active, int m, int tiles_total,
-                           int tps, int JL, double *out, size_t cstride, size_t sstride)
+                           int tps, int JL, double *out, size_t cstride, size_t sstride, bool no_snap)
 {
     const double *jstream = ctx->jp + (size_t)ctx->j_begin * REC;   // j-shard (nb_set_j_range), else the whole stream
 #define NB_KF(G0, MXP)                                                                 \
     k_force<NT, TJ, MINB, JLT, G0, MXP><<<grid, NT, 0, ctx->stream>>>(ctx->jp, jstream, active, m, tiles_total, tps, JL, \
                                                                       ctx->eps2, out, cstride, sstride)
     const bool g0 = ctx->eps == 0.0, mx = ctx->precision == 1;
-    if (g0 && mx) NB_KF(true, true);
-    else if (g0) NB_KF(true, false);
-    else if (mx) NB_KF(false, true);
-    else NB_KF(false, false);
+    if (g0 && mx) NB_KF(true, 1);
+    else if (mx) NB_KF(false, 1);
+    else if (g0 && no_snap) NB_KF(true, 2);
+    else if (no_snap) NB_KF(false, 2);
+    else if (g0) NB_KF(true, 0);
+    else NB_KF(false, 0);
 #undef NB_KF
 }
 
-int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m)
+int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m, bool no_snap)
 {
     if (m <= 0) return NB_OK;
     // records of the j-shard, padded to whole tiles (records N..Npad-1 have zero mass)
@@ -490,9 +497,9 @@ int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m)
     }
     dim3 grid((unsigned)g.n_ib, (unsigned)g.S, 1);
     if (varA)
-        launch_variant<NT_A, TJ_A, MINB_A, 1>(ctx, grid, active, (int)m, (int)tiles, g.tps, 1, out, cstride, sstride);
+        launch_variant<NT_A, TJ_A, MINB_A, 1>(ctx, grid, active, (int)m, (int)tiles, g.tps, 1, out, cstride, sstride, no_snap);
     else
-        launch_variant<NT_B, TJ_B, MINB_B, 0>(ctx, grid, active, (int)m, (int)tiles, g.tps, g.JL, out, cstride, sstride);
+        launch_variant<NT_B, TJ_B, MINB_B, 0>(ctx, grid, active, (int)m, (int)tiles, g.tps, g.JL, out, cstride, sstride, no_snap);
     NB_LAUNCH_CHECK(ctx, "k_force");
     if (g.S > 1) {
         if (g.S < 32) {
@@ -525,10 +532,10 @@ int enqueue_force_persistent(nb_ctx *ctx, int parity)
             ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);            \
     } while (0)
     const bool g0 = ctx->eps == 0.0, mx = ctx->precision == 1;
-    if (g0 && mx) NB_KP(true, true);
-    else if (g0) NB_KP(true, false);
-    else if (mx) NB_KP(false, true);
-    else NB_KP(false, false);
+    if (g0 && mx) NB_KP(true, 1);
+    else if (g0) NB_KP(true, 0);
+    else if (mx) NB_KP(false, 1);
+    else NB_KP(false, 0);
 #undef NB_KP
     NB_LAUNCH_CHECK(ctx, "k_force_persistent");
     ctx->n_launch += 1;  // two kernels

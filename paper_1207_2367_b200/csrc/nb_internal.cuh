@@ -207,7 +207,7 @@ namespace nb {
 // Evaluate (acc, jerk, snap) of `m` particles (active == nullptr: particles 0..m-1) against the
 // Npad predicted records; result in ctx->f1[c][k].  with_snap = false skips nothing in the
 // arithmetic (the body is the same); it only exists for symmetry of the start-up passes.
-int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m);
+int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m, bool no_snap = false);
 int query_force_occupancy(nb_ctx *ctx);
 int enqueue_force_persistent(nb_ctx *ctx, int parity);   // both variants; the selected one chooses the geometry
 // f1[c][k] -> out[q][k][3] (q = 0 acc, 1 jerk, 2 snap) contiguous in ctx->stage
