@@ -118,3 +118,19 @@ def test_graph_loop_matches_oracle_config1_quarter(nb, oracle):
     err = (np.linalg.norm(r - it.pos, axis=1) / np.linalg.norm(it.pos, axis=1)).max()
     assert err < 1e-9
     g.close()
+
+
+def test_graph_loop_large_ragged_n(nb):
+    """N = 150 001 (not a multiple of any tile), batch of 64 steps replayed over many scheduler blocks; the
+    first steps have m from a handful to tens of thousands: both evaluation variants, S > 1 and S = 1."""
+    n = 150001
+    pos, vel, m = plummer(n, seed=24)
+    a = _mk(nb, pos, vel, m, 1e-3, 0.45, 2.0 ** -25, 2.0 ** -4, graph=True)
+    b = _mk(nb, pos, vel, m, 1e-3, 0.45, 2.0 ** -25, 2.0 ** -4, graph=False)
+    a.run_steps(12, log=False)
+    b.run_steps(12, log=False)
+    sa, sb = a.stats(), b.stats()
+    assert sa["n_steps"] == sb["n_steps"] == 12 and sa["n_pairs"] == sb["n_pairs"] and sa["t_now"] == sb["t_now"]
+    assert list(sa["hist"]) == list(sb["hist"]) and sa["hist"][4:].sum() > 0      # some large blocks among them
+    assert np.array_equal(_full(nb, a, n), _full(nb, b, n))
+    a.close(); b.close()
