@@ -520,9 +520,8 @@ int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m, bool no_snap)
 // Device-driven loop: both variants are enqueued with fixed grids (one wave of resident CTAs);
 // the one the gather kernel did not select returns at once, as does everything when the control
 // block says `done`.
-int enqueue_force_persistent(nb_ctx *ctx, int parity)
+int enqueue_force_persistent(nb_ctx *ctx)
 {
-    (void)parity;  // the set size and geometry come from the control block
     const unsigned gA = (unsigned)(ctx->n_sm * ctx->occ[2]), gB = (unsigned)(ctx->n_sm * ctx->occ[3]);
 #define NB_KP(G0, MXP)                                                                                       \
     do {                                                                                                     \

@@ -209,7 +209,7 @@ namespace nb {
 // arithmetic (the body is the same); it only exists for symmetry of the start-up passes.
 int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m, bool no_snap = false);
 int query_force_occupancy(nb_ctx *ctx);
-int enqueue_force_persistent(nb_ctx *ctx, int parity);   // both variants; the selected one chooses the geometry
+int enqueue_force_persistent(nb_ctx *ctx);   // both variants + reduction; set size and geometry come from ctx->ctl
 // f1[c][k] -> out[q][k][3] (q = 0 acc, 1 jerk, 2 snap) contiguous in ctx->stage
 int launch_unpack_f1(nb_ctx *ctx, int64_t m);
 int launch_f1_contig(nb_ctx *ctx, int64_t m, double *buf, bool to_f1);
