@@ -1,8 +1,9 @@
 // nb_energy.cu -- diagnostics: E = K + W with the softened pair potential of Eq. 2
 // (PAPER.md:40), total momentum and angular momentum (Eq. 20), computed from the
 // predicted stream (positions and velocities at the current time).
-//   W = -1/2 sum_i m_i sum_{j != i} m_j / sqrt(|r_ij|^2 + eps^2)   (the j = i term is skipped
-//   by index: with eps > 0 it is NOT zero)
+//   W = -sum_i m_i sum_{j > i} m_j / sqrt(|r_ij|^2 + eps^2)   (every pair once, as Eq. 2 is
+//   written; the j = i term is excluded by index: with eps > 0 it is NOT zero).  Thread i sums
+//   over j > i only, so the blocks have triangular work (the block scheduler balances them).
 // Reductions are fixed-order trees, so the result is bit-reproducible.
 #include "nb_internal.cuh"
 
@@ -10,6 +11,7 @@ namespace nb {
 
 constexpr int EN_THREADS = 128;
 constexpr int EN_TJ = 128;
+static_assert(EN_THREADS == EN_TJ, "the triangular loop starts at the block's own tile");
 
 __device__ __forceinline__ double rsqrt_full(double s)
 {
@@ -45,7 +47,8 @@ __global__ void __launch_bounds__(EN_THREADS)
     const double xi = pi[0], yi = pi[1], zi = pi[2], vx = pi[3], vy = pi[4], vz = pi[5];
     const double mi = live ? pi[9] : 0.0;
     double pot = 0.0;
-    for (int64_t j0 = 0; j0 < Npad; j0 += EN_TJ) {
+    // first tile that holds a j > i for some i of this block (blocks and tiles are both 128 long)
+    for (int64_t j0 = (int64_t)blockIdx.x * EN_THREADS; j0 < Npad; j0 += EN_TJ) {
         __syncthreads();
         {
             const double *pj = jp + (j0 + threadIdx.x) * REC;
@@ -63,14 +66,16 @@ __global__ void __launch_bounds__(EN_THREADS)
             const double dx = a.x - xi, dy = a.y - yi, dz = b.x - zi;
             const double s = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
             double y = rsqrt_full(s);
-            if (j0 + jj == i || b.y == 0.0) y = 0.0;  // self term; padded / massless records
+            // pairs with j <= i belong to the other particle's sum; padded / massless records add
+            // nothing (integer test on the bits: +0.0 only, no FP64 pipe slot)
+            if (j0 + jj <= i || __double_as_longlong(b.y) == 0) y = 0.0;
             p = fma(b.y, y, p);
         }
         pot += p;
     }
     double vals[8];
     vals[0] = 0.5 * mi * (vx * vx + vy * vy + vz * vz);
-    vals[1] = -0.5 * mi * pot;
+    vals[1] = -mi * pot;
     vals[2] = mi * vx; vals[3] = mi * vy; vals[4] = mi * vz;
     vals[5] = mi * (yi * vz - zi * vy);
     vals[6] = mi * (zi * vx - xi * vz);
