@@ -37,6 +37,7 @@ static void release(nb_ctx *ctx)
     graph_release(ctx);
     if (ctx->h_ctl) cudaFreeHost(ctx->h_ctl);
     if (ctx->ctl) cudaFree(ctx->ctl);
+    if (ctx->geom_cache) cudaFree(ctx->geom_cache);
     void *bufs[] = {ctx->mass, ctx->t, ctx->dt, ctx->r, ctx->v, ctx->a, ctx->j, ctx->s, ctx->c, ctx->jp,
                     ctx->active, ctx->user_idx, ctx->f1, ctx->stage, ctx->partials, ctx->d_tmin,
                     ctx->blk_count, ctx->red};
@@ -117,7 +118,8 @@ extern "C" int nb_init(nb_ctx **out, int64_t N, const double *pos, const double 
     if (cudaHostAlloc((void **)&ctx->h_sched, sizeof(Sched), cudaHostAllocMapped) != cudaSuccess) return fail(NB_ENOMEM);
     if (cudaHostGetDevicePointer((void **)&ctx->d_sched, ctx->h_sched, 0) != cudaSuccess) return fail(NB_ECUDA);
     ctx->h_sched->t_next = 0.0; ctx->h_sched->n_active = 0;
-    if ((rc = dev_alloc(ctx, &ctx->ctl, 1))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->ctl, 1)) || (rc = dev_alloc(ctx, &ctx->geom_cache, (size_t)GEOM_CACHE_M + 1)))
+        return fail(rc);
     if (cudaHostAlloc((void **)&ctx->h_ctl, sizeof(StepCtl), cudaHostAllocDefault) != cudaSuccess) return fail(NB_ENOMEM);
     memset(ctx->h_ctl, 0, sizeof(StepCtl));
     ctx->use_graph = 1;
@@ -151,6 +153,9 @@ extern "C" int nb_startup(nb_ctx *ctx)
 {
     if (!ctx) return NB_EINVAL;
     if (ctx->started) return set_err(ctx, NB_ESTATE, "nb_startup: already started");
+    // a context that steps will split small active sets over many j-pieces: take the partial-sum buffer
+    // now (up to 0.5 GB at large N) rather than inside the first block step
+    NB_TRY(reserve_partials(ctx, ctx->partials_limit));
     // predicted stream <- (r, v, a = 0) at t = 0 (all t_i = 0, derivatives 0: the predictor is the identity)
     NB_TRY(launch_predict(ctx, 0.0));
     NB_TRY(launch_force(ctx, nullptr, ctx->N, true)); // pass 1: a, jerk only (its snap would lack the m da term)

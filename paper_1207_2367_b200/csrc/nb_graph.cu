@@ -50,6 +50,8 @@ static int build_graph(nb_ctx *ctx)
     ctx->n_launch = launches;  // captured, not launched
     cudaStreamDestroy(cap);
     if (rc != NB_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+    // the remembered geometries belong to the knobs this graph is captured with
+    NB_CUDA(ctx, cudaMemsetAsync(ctx->geom_cache, 0, ((size_t)GEOM_CACHE_M + 1) * sizeof(ForceGeom), ctx->stream));
     const cudaError_t e3 = cudaGraphInstantiate(&ctx->step_graph, graph, 0);
     cudaGraphDestroy(graph);
     if (e3 != cudaSuccess) return set_err(ctx, NB_ECUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e3));

@@ -56,6 +56,7 @@ struct StepCtl {
 constexpr int NT_A = 128, TJ_A = 128, MINB_A = 4;   // variant A: one i per thread, m >= 128
 constexpr int NT_B = 32, TJ_B = 64, MINB_B = 16;    // variant B: one warp per CTA, small m
 constexpr int64_t L2_CHUNK_BYTES = 24 << 20;         // j-stream piece kept L2-resident across i-block waves
+constexpr int GEOM_CACHE_M = 4096;                   // the device loop remembers the geometry of set sizes up to this
 constexpr int MAX_WAVES = 64;                       // the split search considers 1..MAX_WAVES waves
 
 // Number of j-splits.  All CTAs do the same work per tile, so the cost of a launch is
@@ -179,6 +180,7 @@ struct nb_ctx {
     nb::Sched *d_sched;             // device alias of h_sched
     nb::StepCtl *ctl;               // device control block of the graph-driven block-step loop
     nb::StepCtl *h_ctl;             // pinned host copy, refreshed after every graph launch
+    nb::ForceGeom *geom_cache;      // [GEOM_CACHE_M + 1], S == 0: not computed yet (device loop only)
     cudaGraphExec_t step_graph;     // `graph_batch` block steps captured once per context
     int graph_batch;
     int graph_split, graph_jlanes, graph_precision;  // knobs the captured graph was built with
