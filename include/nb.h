@@ -185,8 +185,11 @@ int nb_set_forces(nb_ctx *ctx, const double *buf);
 int nb_set_precision(nb_ctx *ctx, int mode);
 
 /* Driver of nb_run_until / nb_run_steps: 1 (default) = device-driven CUDA-graph batches,
- * 0 = the host issues nb_next_block / nb_predict / nb_force / nb_correct_and_step per step.
- * Both give bit-identical states.  nb_run_steps with a per-step log always uses 0.          */
+ * 2 = the same graph with its kernels chained by programmatic dependent launch (each kernel is
+ * launched while its predecessor still runs and waits on the device for its completion; measured
+ * slower than plain graph edges on B200, kept for comparison), 0 = the host issues nb_next_block /
+ * nb_predict / nb_force / nb_correct_and_step per step.  All give bit-identical states.
+ * nb_run_steps with a per-step log always uses 0.                                           */
 int nb_set_loop_mode(nb_ctx *ctx, int device_driven);
 
 /* What the last nb_force launched: out [host] = {threads per CTA, j-lanes per i, j-splits,

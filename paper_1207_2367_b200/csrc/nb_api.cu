@@ -475,7 +475,7 @@ extern "C" int nb_set_precision(nb_ctx *ctx, int mode)
 extern "C" int nb_set_loop_mode(nb_ctx *ctx, int device_driven)
 {
     if (!ctx) return NB_EINVAL;
-    if (device_driven != 0 && device_driven != 1) return set_err(ctx, NB_EINVAL, "nb_set_loop_mode: 0 or 1");
+    if (device_driven < 0 || device_driven > 2) return set_err(ctx, NB_EINVAL, "nb_set_loop_mode: 0, 1 or 2");
     ctx->use_graph = device_driven;
     return NB_OK;
 }

@@ -317,6 +317,8 @@ __global__ void __launch_bounds__(NT, MINB)
                        const int64_t Npad, const double eps2, double *__restrict__ f1,
                        double *__restrict__ partials, const StepCtl *__restrict__ ctl)
 {
+    pdl_trigger();
+    pdl_wait();
     if (ctl->done || ctl->g.variant != (JLT ? 0 : 1)) return;
     __shared__ __align__(128) double tile[2][TJ * REC];
     __shared__ __align__(8) uint64_t full[2];
@@ -390,6 +392,8 @@ __global__ void __launch_bounds__(256)
     k_reduce_persistent(const double *__restrict__ part, const StepCtl *__restrict__ ctl, double *__restrict__ f1,
                         const size_t f1stride)
 {
+    pdl_trigger();
+    pdl_wait();
     if (ctl->done || ctl->g.S <= 1) return;
     const int S = ctl->g.S, m = (int)ctl->n_active;
     const size_t cstride = (size_t)ctl->g.mpad, sstride = 9 * (size_t)ctl->g.mpad;
@@ -525,12 +529,12 @@ int enqueue_force_persistent(nb_ctx *ctx)
     const unsigned gA = (unsigned)(ctx->n_sm * ctx->occ[2]), gB = (unsigned)(ctx->n_sm * ctx->occ[3]);
 #define NB_KP(G0, MXP)                                                                                       \
     do {                                                                                                     \
-        k_force_persistent<NT_A, TJ_A, MINB_A, 1, G0, MXP><<<gA, NT_A, 0, ctx->stream>>>(                      \
-            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);            \
-        k_force_persistent<NT_B, TJ_B, MINB_B, 0, G0, MXP><<<gB, NT_B, 0, ctx->stream>>>(                      \
-            ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);            \
+        launch_chain(k_force_persistent<NT_A, TJ_A, MINB_A, 1, G0, MXP>, dim3(gA), dim3(NT_A), ctx->stream, pdl, \
+                     ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);   \
+        launch_chain(k_force_persistent<NT_B, TJ_B, MINB_B, 0, G0, MXP>, dim3(gB), dim3(NT_B), ctx->stream, pdl, \
+                     ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);   \
     } while (0)
-    const bool g0 = ctx->eps == 0.0, mx = ctx->precision == 1;
+    const bool g0 = ctx->eps == 0.0, mx = ctx->precision == 1, pdl = ctx->use_graph == 2;
     if (g0 && mx) NB_KP(true, 1);
     else if (g0) NB_KP(true, 0);
     else if (mx) NB_KP(false, 1);
@@ -538,7 +542,8 @@ int enqueue_force_persistent(nb_ctx *ctx)
 #undef NB_KP
     NB_LAUNCH_CHECK(ctx, "k_force_persistent");
     ctx->n_launch += 1;  // two kernels
-    k_reduce_persistent<<<(unsigned)(2 * ctx->n_sm), 256, 0, ctx->stream>>>(ctx->partials, ctx->ctl, ctx->f1, (size_t)ctx->Npad);
+    launch_chain(k_reduce_persistent, dim3((unsigned)(2 * ctx->n_sm)), dim3(256), ctx->stream, pdl, ctx->partials,
+                 ctx->ctl, ctx->f1, (size_t)ctx->Npad);
     NB_LAUNCH_CHECK(ctx, "k_reduce_persistent");
     return NB_OK;
 }

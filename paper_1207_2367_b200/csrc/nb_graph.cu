@@ -58,6 +58,7 @@ static int build_graph(nb_ctx *ctx)
     ctx->graph_batch = B;
     ctx->graph_split = ctx->force_split; ctx->graph_jlanes = ctx->force_jlanes;
     ctx->graph_precision = ctx->precision;
+    ctx->graph_pdl = ctx->use_graph == 2;
     return NB_OK;
 }
 
@@ -72,7 +73,7 @@ int graph_run(nb_ctx *ctx, double t_end, int64_t max_steps, int64_t *n_steps)
 {
     // tuning knobs are kernel arguments of the captured nodes: re-capture when they changed
     if (ctx->step_graph && (ctx->graph_split != ctx->force_split || ctx->graph_jlanes != ctx->force_jlanes ||
-                            ctx->graph_precision != ctx->precision))
+                            ctx->graph_precision != ctx->precision || ctx->graph_pdl != (ctx->use_graph == 2)))
         graph_release(ctx);
     {
         const int rc = reserve_partials(ctx, ctx->partials_limit);  // no allocation inside a replay

@@ -53,6 +53,30 @@ struct StepCtl {
     long long hist[64];
 };
 
+#ifdef __CUDACC__
+// Programmatic dependent launch (sm_90+, PTX griddepcontrol), loop mode 2: the kernels of the
+// device-driven loop are launched with cudaLaunchAttributeProgrammaticStreamSerialization, let their
+// successor start launching at once (pdl_trigger) and wait for the COMPLETION of their predecessor
+// (pdl_wait: all its blocks done, its writes visible) before they read anything it wrote.  Every
+// kernel of the chain waits, so completion is transitive; without the launch attribute (mode 1, the
+// default: plain graph edges measured faster) both are no-ops.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_chain(void (*kern)(KArgs...), dim3 grid, dim3 block, cudaStream_t stream, bool pdl,
+                                Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = 0; cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+#endif
+
 constexpr int NT_A = 128, TJ_A = 128, MINB_A = 4;   // variant A: one i per thread, m >= 128
 constexpr int NT_B = 32, TJ_B = 64, MINB_B = 16;    // variant B: one warp per CTA, small m
 constexpr int64_t L2_CHUNK_BYTES = 24 << 20;         // j-stream piece kept L2-resident across i-block waves
@@ -185,7 +209,8 @@ struct nb_ctx {
     int graph_batch;
     int graph_split, graph_jlanes, graph_precision;  // knobs the captured graph was built with
     int64_t launches_per_batch;     // kernels in one replay of step_graph
-    int use_graph;                  // 1: nb_run_until / nb_run_steps drive the loop from the device
+    int use_graph;                  // 1, 2: nb_run_until / nb_run_steps drive the loop from the device (2: with PDL)
+    int graph_pdl;                  // the captured graph uses programmatic dependent launch
 
     // tuning
     int force_split, force_jlanes;

@@ -574,6 +574,8 @@ __global__ void __launch_bounds__(SCHED_THREADS)
                        const int occB, const int64_t partials_limit, const int force_split, const int force_jlanes,
                        ForceGeom *__restrict__ geom_cache)
 {
+    pdl_trigger();
+    pdl_wait();
     // every block evaluates the same condition from values no kernel of this step modifies
     const double tn = __longlong_as_double((long long)ctl->tmin[p]);
     const bool done = ctl->done || ctl->steps_left <= 0 || !(tn <= ctl->t_end);
@@ -663,6 +665,8 @@ __global__ void __launch_bounds__(SCHED_THREADS)
                        double *__restrict__ dti, double *__restrict__ r, double *__restrict__ v,
                        double *__restrict__ a, double *__restrict__ j, double *__restrict__ s, double *__restrict__ c)
 {
+    pdl_trigger();
+    pdl_wait();
     if (ctl->done) return;
     const int m = (int)ctl->n_active;
     const double tn = ctl->t_next;
@@ -700,11 +704,10 @@ int launch_graph_begin(nb_ctx *ctx, double t_end, int64_t steps)
 int enqueue_graph_gather_predict(nb_ctx *ctx, int parity)
 {
     const unsigned np = (unsigned)((ctx->N + SCHED_THREADS - 1) / SCHED_THREADS);
-    k_g_gather_predict<<<np, SCHED_THREADS, 0, ctx->stream>>>(parity, ctx->N, ctx->Npad, ctx->t, ctx->dt, ctx->active,
-                                                               ctx->ctl, ctx->mass, ctx->r, ctx->v, ctx->a, ctx->j,
-                                                               ctx->s, ctx->c, ctx->jp, ctx->n_sm, ctx->occ[0], ctx->occ[1],
-                                                               (int64_t)ctx->partials_limit, ctx->force_split,
-                                                               ctx->force_jlanes, ctx->geom_cache);
+    launch_chain(k_g_gather_predict, dim3(np), dim3(SCHED_THREADS), ctx->stream, ctx->use_graph == 2, parity, ctx->N,
+                 ctx->Npad, ctx->t, ctx->dt, ctx->active, ctx->ctl, ctx->mass, ctx->r, ctx->v, ctx->a, ctx->j, ctx->s,
+                 ctx->c, ctx->jp, ctx->n_sm, ctx->occ[0], ctx->occ[1], (int64_t)ctx->partials_limit, ctx->force_split,
+                 ctx->force_jlanes, ctx->geom_cache);
     NB_LAUNCH_CHECK(ctx, "k_g_gather_predict");
     return NB_OK;
 }
@@ -713,10 +716,9 @@ int enqueue_graph_correct(nb_ctx *ctx, int parity)
 {
     int64_t g = (ctx->N + SCHED_THREADS - 1) / SCHED_THREADS;
     if (g > 4 * ctx->n_sm) g = 4 * ctx->n_sm;
-    k_g_correct<<<(unsigned)g, SCHED_THREADS, 0, ctx->stream>>>(parity, ctx->N, ctx->Npad, ctx->active, ctx->ctl,
-                                                                      ctx->eta, ctx->dt_min, ctx->dt_max,
-                                                                      ctx->f1, ctx->t, ctx->dt, ctx->r, ctx->v, ctx->a,
-                                                                      ctx->j, ctx->s, ctx->c);
+    launch_chain(k_g_correct, dim3((unsigned)g), dim3(SCHED_THREADS), ctx->stream, ctx->use_graph == 2, parity, ctx->N,
+                 ctx->Npad, ctx->active, ctx->ctl, ctx->eta, ctx->dt_min, ctx->dt_max, ctx->f1, ctx->t, ctx->dt, ctx->r,
+                 ctx->v, ctx->a, ctx->j, ctx->s, ctx->c);
     NB_LAUNCH_CHECK(ctx, "k_g_correct");
     return NB_OK;
 }

@@ -211,7 +211,7 @@ def main():
     ap.add_argument("--etas", default="0.3,0.45,0.6,0.8,1.0")
     ap.add_argument("--ns", default=None, help="comma-separated N list for --experiment fig1")
     ap.add_argument("--heavy-frac", type=float, default=0.05)
-    ap.add_argument("--loop", type=int, default=None, choices=[0, 1], help="0: host-driven loop, 1: device-driven (default)")
+    ap.add_argument("--loop", type=int, default=None, choices=[0, 1, 2], help="0: host-driven loop, 1: device-driven graph batches (default), 2: the same with programmatic dependent launch")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"],
                     help="evaluation arithmetic: fp64 (default) or the paper's mixed SP/DP scheme (PAPER.md:287)")
     a = ap.parse_args()

@@ -18,8 +18,10 @@ pytestmark = pytest.mark.gpu
 
 
 def _mk(nb, pos, vel, m, eps, eta, dt_min, dt_max, graph):
+    """graph: False/0 = host-issued calls, True/1 = CUDA-graph batches (the default), 2 = graph
+    batches whose kernels are chained by programmatic dependent launch."""
     g = nb.NBody(dev(pos), dev(vel), dev(m), eps, eta, dt_min=dt_min, dt_max=dt_max)
-    nb.nb_set_loop_mode(g.ctx, 1 if graph else 0)
+    nb.nb_set_loop_mode(g.ctx, int(graph))
     return g
 
 
@@ -30,10 +32,11 @@ def _full(nb, g, n):
     return host(st)
 
 
+@pytest.mark.parametrize("mode", [1, 2])
 @pytest.mark.parametrize("n,seed,eps,t_end", [(1024, 1, 1e-3, 0.25), (3000, 8, 1e-3, 0.0625), (77, 5, 1e-2, 0.5)])
-def test_graph_loop_is_bit_identical_to_call_sequence(nb, n, seed, eps, t_end):
+def test_graph_loop_is_bit_identical_to_call_sequence(nb, n, seed, eps, t_end, mode):
     pos, vel, m = plummer(n, seed=seed)
-    a = _mk(nb, pos, vel, m, eps, 0.45, 2.0 ** -25, 2.0 ** -4, graph=True)
+    a = _mk(nb, pos, vel, m, eps, 0.45, 2.0 ** -25, 2.0 ** -4, graph=mode)
     b = _mk(nb, pos, vel, m, eps, 0.45, 2.0 ** -25, 2.0 ** -4, graph=False)
     na = a.run_until(t_end)
     nb_ = b.run_until(t_end)
