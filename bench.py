@@ -33,8 +33,8 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the evaluation kernel per launch, from the ncu capture
-# recorded in profiles/r1_bench_launches.md (bench.py cannot run under ncu itself); keyed by N
-NCU_DRAM_BYTES_PER_LAUNCH = {1 << 20: 320013056 + 278509568}
+# in profiles/r1_k_force_ncu_full_N2p20.md (bench.py cannot run under ncu itself); keyed by N
+NCU_DRAM_BYTES_PER_LAUNCH = {1 << 20: 318370048 + 282368000}
 FLOPS_PER_PAIR = 85.0        # 32 DFMA x 2 + 11 DMUL + 10 DADD, counted in the SASS
 FLOPS_PER_PAIR_PAPER = 97.0  # the paper's convention (Table 2)
 # FP64 ALU peak derived from unit counts and clocks: 148 SMs x 64 FP64
@@ -329,7 +329,7 @@ def run_ours(args):
             "roofline": {"bound": "alu", "kernel": "k_force<128,128,4,1>", "achieved": achieved,
                          "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
                          "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(N), "traffic_unit": "bytes per launch (dram__bytes_read.sum + "
-                         "dram__bytes_write.sum, profiles/r1_bench_launches.md); algorithmic 4.70e8",
+                         "dram__bytes_write.sum of the ncu --set full capture in profiles/r1_k_force_ncu_full_N2p20.md); algorithmic 4.70e8",
                          "kernel_ms": kern_ms, "launch": "grid 8192 x 4 splits, 128 threads; + k_reduce_thread" if N == 1 << 20 else None,
                          "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md section 7); "
                                         "MEASURED_PEAKS.json has no FP64 entry",
