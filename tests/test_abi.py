@@ -60,3 +60,21 @@ def test_product_never_imports_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, f)).read()
                 assert "oracle" not in txt.lower(), (dirpath, f)
+
+
+def test_paper_flop_convention_is_consistent():
+    """tests/golden/paper_flop_convention.txt: the printed counts add up, Eq. 27 gives the
+    printed mixed peak, and bench.py quotes Tflop/s in exactly that convention."""
+    import os
+    vals = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_flop_convention.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                k, v = line.split()
+                vals[k] = float(v)
+    assert vals["dp_ops_per_pair"] + vals["sp_ops_per_pair"] == vals["flops_per_pair"] == 97
+    r_peak = (vals["sp_ops_per_pair"] * vals["S_peak_gflops"] + vals["dp_ops_per_pair"] * vals["D_peak_gflops"]) / vals["flops_per_pair"]
+    assert abs(r_peak - vals["R_peak_gflops"]) < 1.0                       # Eq. 27: "~950 GFLOPS"
+    assert abs(vals["reported_gflops_per_gpu"] / r_peak - 0.42) < 0.03      # "around 40% of the claimed peak"
+    import bench
+    assert bench.FLOPS_PER_PAIR_PAPER == vals["flops_per_pair"]

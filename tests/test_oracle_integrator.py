@@ -173,6 +173,17 @@ def test_block_step_invariants(oracle):
     assert len(seen_levels) >= 3
 
 
+def _paper_fig1_band():
+    import os
+    out = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_fig1_energy_errors.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                eta, q, _, val = line.split()
+                out[(float(eta), q)] = float(val)
+    return out
+
+
 def test_energy_error_scales_with_eta(oracle):
     pos, vel, m = plummer(256, seed=1)
     errs = {}
@@ -185,7 +196,11 @@ def test_energy_error_scales_with_eta(oracle):
     assert errs[0.1] < errs[0.2] < errs[0.45]
     slope = math.log(errs[0.45] / errs[0.1]) / math.log(4.5)
     assert 3.0 < slope < 7.5, (errs, slope)
-    assert errs[0.45] < 1e-6            # plausibility band of PAPER.md:141 (eta ~ 0.45-0.6)
+    # plausibility band from the values the paper prints (tests/golden/paper_fig1_energy_errors.txt,
+    # PAPER.md:141): below 5e-9 at eta = 0.6 for N >= 2^15 in mixed precision; a 256-body FP64 run at the
+    # smaller eta = 0.45 must not be two orders of magnitude worse than that, nor below the paper's floor
+    band = _paper_fig1_band()
+    assert band[(0.3, "dE_over_E")] < errs[0.45] < 100 * band[(0.6, "dE_over_E")]
 
 
 # ---------------------------------------------------------------- energy (Eq. 2, Eq. 20)
