@@ -52,31 +52,43 @@ __device__ __forceinline__ void pair_body(const double xi, const double yi, cons
     const double2 p2 = *reinterpret_cast<const double2 *>(q + 4);
     const double2 p3 = *reinterpret_cast<const double2 *>(q + 6);
     const double2 p4 = *reinterpret_cast<const double2 *>(q + 8);
-    const double dx = p0.x - xi, dy = p0.y - yi, dz = p1.x - zi;
-    const double dvx = p1.y - vxi, dvy = p2.x - vyi, dvz = p2.y - vzi;
-    const double dax = p3.x - axi, day = p3.y - ayi, daz = p4.x - azi;
+    // differences and the three dot products, component by component (z, y, x)
+    const double dvz = p2.y - vzi, dvy = p2.x - vyi, dvx = p1.y - vxi;
+    double vr = dvz * dvz;
+    vr = fma(dvy, dvy, vr);
+    vr = fma(dvx, dvx, vr);
+    const double dz = p1.x - zi, daz = p4.x - azi;
+    double s = fma(dz, dz, eps2);
+    double rv = dz * dvz;
+    vr = fma(dz, daz, vr);
+    const double dy = p0.y - yi, day = p3.y - ayi;
+    s = fma(dy, dy, s);
+    rv = fma(dy, dvy, rv);
+    vr = fma(dy, day, vr);
+    const double dx = p0.x - xi, dax = p3.x - axi;
+    s = fma(dx, dx, s);
+    rv = fma(dx, dvx, rv);
+    vr = fma(dx, dax, vr);
     const double mj = p4.y;
-    const double s = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
-    const double rv = fma(dx, dvx, fma(dy, dvy, dz * dvz));
-    const double vr = fma(dx, dax, fma(dy, day, fma(dz, daz, fma(dvx, dvx, fma(dvy, dvy, dvz * dvz)))));
     double y0 = rsqrt_seed(s);
     if (GUARD0) {  // eps = 0: a coincident pair (the self term) contributes nothing (G12)
         if ((__double2hiint(s) | __double2loint(s)) == 0) y0 = 0.0;
     }
+    // y = y0 (1 + e (1/2 + 3/8 e)), e = 1 - s y0^2: every instruction reads at most two registers
     const double y2 = y0 * y0;
     const double e = fma(-s, y2, 1.0);
-    const double p = fma(0.375, e, 0.5);
-    const double ye = y0 * e;
-    const double y = fma(ye, p, y0);   // s^(-1/2)
+    const double p = fma(e, 0.375, 0.5);
+    const double ep1 = fma(e, p, 1.0);
+    const double y = y0 * ep1;         // s^(-1/2)
     const double ri2 = y * y;          // 1/s
     const double my = mj * y;
+    const double qq = ri2 * -3.0;
     const double w = my * ri2;         // m_j s^(-3/2)
-    const double qq = -3.0 * ri2;
     const double g = rv * qq;          // -3 alpha
-    const double al = g * (-1.0 / 3.0);
     const double qv = qq * vr;
-    const double b3 = fma(al, g, qv);  // -3 beta = -3 (v^2 + r.a)/s - 3 alpha^2
+    const double gg = g * g;
     const double g2 = g + g;
+    const double b3 = fma(gg, -1.0 / 3.0, qv);  // -3 beta = -3 (v^2 + r.a)/s - 3 alpha^2
     const double ux = fma(g, dx, dvx), uy = fma(g, dy, dvy), uz = fma(g, dz, dvz);
     A.ax = fma(w, dx, A.ax);
     A.ay = fma(w, dy, A.ay);
@@ -231,7 +243,7 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
                 AccF A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
                 const float eps2f = (float)eps2;
                 if (JLT) {
-#pragma unroll UNR
+#pragma unroll 4
                     for (int jj = 0; jj < TJ; ++jj)
                         pair_body_mx<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2f, A);
                 } else {
@@ -288,7 +300,7 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
 }
 
 // grid.x: i-blocks, grid.y: j-splits; geometry passed by the host.
-template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int MX = 0, int UNR = 4>
+template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int MX = 0, int UNR = 12>
 __global__ void __launch_bounds__(NT, MINB)
     k_force(const double *__restrict__ jp, const double *__restrict__ jstream,
             const int32_t *__restrict__ active, const int m, const int tiles_total, const int tiles_per_split, const int JLr, const double eps2,
@@ -311,7 +323,7 @@ __global__ void __launch_bounds__(NT, MINB)
 // resident CTAs; the set size and the geometry are read from the control block, where the gather
 // kernel of the same step left them; CTA b takes the work items b, b + gridDim.x, ...  Item w is
 // (i-block w % n_ib, split w / n_ib), so concurrently running CTAs stream the same j-split.
-template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int MX = 0, int UNR = 4>
+template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int MX = 0, int UNR = 12>
 __global__ void __launch_bounds__(NT, MINB)
     k_force_persistent(const double *__restrict__ jp, const int32_t *__restrict__ active_list, const int64_t N,
                        const int64_t Npad, const double eps2, double *__restrict__ f1,
