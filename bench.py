@@ -34,7 +34,7 @@ if ROOT not in sys.path:
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the evaluation kernel per launch, from the ncu capture
 # in profiles/r1_k_force_ncu_full_N2p20.md (bench.py cannot run under ncu itself); keyed by N
-NCU_DRAM_BYTES_PER_LAUNCH = {1 << 20: 318370048 + 282368000}
+NCU_DRAM_BYTES_PER_LAUNCH = {1 << 20: 384024320 + 450180352}
 FLOPS_PER_PAIR = 85.0        # 32 DFMA x 2 + 11 DMUL + 10 DADD, counted in the SASS
 FLOPS_PER_PAIR_PAPER = 97.0  # the paper's convention (Table 2)
 # FP64 ALU peak derived from unit counts and clocks: 148 SMs x 64 FP64
