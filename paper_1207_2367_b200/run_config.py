@@ -54,9 +54,18 @@ def run_integration(nb, cfg, c, N, t_end, n_steps, loop=None):
     out = {"config": cfg, "name": c["name"], "N": N, "eps": c["eps"], "eta": c["eta"],
            "startup_s": t_start, "startup_pairs_per_s": 2.0 * N * N / t_start, "E0": float(e0[0])}
     if n_steps:                                   # config 5: a fixed number of block steps
-        lt, lm, ms = g.run_steps(n_steps)
+        st0 = torch.empty((N, 21), dtype=torch.float64, device="cuda")
+        nb.nb_get_full_state(g.ctx, st0); g.sync()
+        lt, lm, ms = g.run_steps(n_steps)         # per-step log: host-issued calls, CUDA events per step
         out["steps"] = [{"t": float(t), "m": int(mm), "ms": float(x), "pairs_per_s": float(mm) * N / (float(x) * 1e-3)}
                         for t, mm, x in zip(lt, lm, ms)]
+        # the same steps again from the same state through the device-driven loop, timed as a whole
+        # (twice: the first run also captures and instantiates the CUDA graph of this context)
+        for _ in range(2):
+            nb.nb_set_full_state(g.ctx, st0); g.sync()
+            t0 = time.perf_counter(); g.run_steps(n_steps, log=False); g.sync(); w = time.perf_counter() - t0
+        out["host_issued_total_ms"] = float(sum(ms))
+        out["device_loop_total_ms"] = w * 1e3
     else:
         t0 = time.perf_counter(); n = g.run_until(t_end); wall = time.perf_counter() - t0
         st = g.stats()
