@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(EN_THREADS)
         }
         __syncthreads();
         double p = 0.0;
-#pragma unroll 8
+#pragma unroll 12
         for (int jj = 0; jj < EN_TJ; ++jj) {
             const double2 a = *reinterpret_cast<const double2 *>(tile + 4 * jj);
             const double2 b = *reinterpret_cast<const double2 *>(tile + 4 * jj + 2);

@@ -243,7 +243,7 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
                 AccF A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
                 const float eps2f = (float)eps2;
                 if (JLT) {
-#pragma unroll 4
+#pragma unroll 6
                     for (int jj = 0; jj < TJ; ++jj)
                         pair_body_mx<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2f, A);
                 } else {
@@ -321,19 +321,22 @@ __global__ void __launch_bounds__(NT, MINB)
 
 // Persistent form for the device-driven block-step loop (nb_graph.cu): a fixed grid of
 // resident CTAs; the set size and the geometry are read from the control block, where the gather
-// kernel of the same step left them; CTA b takes the work items b, b + gridDim.x, ...  Item w is
-// (i-block w % n_ib, split w / n_ib), so concurrently running CTAs stream the same j-split.
+// kernel of the same step left them.  CTA b starts with work item b and then draws the next one
+// from a counter in the control block (items of one launch take equally long, but CTAs do not start
+// together: a fixed stride left a 2 % tail at m ~ 2e5).  Item w is (i-block w % n_ib, split
+// w / n_ib), so concurrently running CTAs stream the same j-split.
 template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int MX = 0, int UNR = 12>
 __global__ void __launch_bounds__(NT, MINB)
     k_force_persistent(const double *__restrict__ jp, const int32_t *__restrict__ active_list, const int64_t N,
                        const int64_t Npad, const double eps2, double *__restrict__ f1,
-                       double *__restrict__ partials, const StepCtl *__restrict__ ctl)
+                       double *__restrict__ partials, StepCtl *__restrict__ ctl)
 {
     pdl_trigger();
     pdl_wait();
     if (ctl->done || ctl->g.variant != (JLT ? 0 : 1)) return;
     __shared__ __align__(128) double tile[2][TJ * REC];
     __shared__ __align__(8) uint64_t full[2];
+    __shared__ long long next_item;
     if (threadIdx.x == 0) {
         mbar_init(&full[0], 1);
         mbar_init(&full[1], 1);
@@ -349,9 +352,15 @@ __global__ void __launch_bounds__(NT, MINB)
     const int tiles_total = (int)(Npad / TJ);
     const long long items = (long long)g.n_ib * g.S;
     unsigned tc = 0;
-    for (long long w = blockIdx.x; w < items; w += gridDim.x)
+    long long w = blockIdx.x;
+    while (w < items) {
         force_item<NT, TJ, JLT, GUARD0, MX, UNR>(jp, jp, active, m, (int)(w % g.n_ib), (int)(w / g.n_ib), tiles_total,
                                                  g.tps, g.JL, eps2, out, cstride, sstride, tile, full, tc);
+        if (threadIdx.x == 0) next_item = (long long)gridDim.x + atomicAdd(&ctl->work, 1u);
+        __syncthreads();
+        w = next_item;
+        __syncthreads();
+    }
 }
 
 // ---- partial-sum reduction (Table 1 row 4): f1[c][k] = sum_s part[s][c][k], s ascending ---

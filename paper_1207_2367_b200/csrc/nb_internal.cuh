@@ -44,6 +44,7 @@ struct StepCtl {
     // collects the minimum for the next step.  cnt[p] = append counter of this step's active list.
     unsigned long long tmin[2];
     int cnt[2];
+    unsigned int work;             // next work item of the persistent evaluation kernel (dynamic distribution)
     int done;                      // set when the next block lies beyond t_end / no steps left
     unsigned int ticket;           // blocks of the gather kernel that have finished (the last one chooses the geometry)
     double t_next, t_end, t_now;

@@ -546,7 +546,7 @@ __global__ void k_g_begin(StepCtl *ctl, const double t_end, const long long step
 {
     ctl->tmin[0] = 0x7ff0000000000000ULL; ctl->tmin[1] = 0x7ff0000000000000ULL;
     ctl->cnt[0] = 0; ctl->cnt[1] = 0;
-    ctl->done = 0; ctl->ticket = 0;
+    ctl->done = 0; ctl->ticket = 0; ctl->work = 0;
     ctl->t_end = t_end; ctl->steps_left = steps; ctl->n_steps = 0; ctl->n_pairs = 0.0;
     for (int b = 0; b < 64; ++b) ctl->hist[b] = 0;
 }
@@ -687,6 +687,7 @@ __global__ void __launch_bounds__(SCHED_THREADS)
         ctl->hist[b] += 1;
         ctl->tmin[p] = 0x7ff0000000000000ULL;   // this step's minimum is consumed: slot p collects the one after next
         ctl->cnt[p] = 0;
+        ctl->work = 0;
     }
 }
 
