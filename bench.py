@@ -57,6 +57,7 @@ def parse():
                     help="step: full block step (default); force: nb_force only (profiling aid)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-block-step", action="store_true", help="skip the block-step wall-time legs (configs 1 and 2)")
     return ap.parse_args()
 
 
@@ -314,6 +315,12 @@ def run_ours(args):
     if rank == 0 and not args.no_cpu_baseline:
         cpu, _, _ = cpu_oracle_sample(pos, vel, accp, m)
 
+    # the other half of BASELINE.json's metric, "block-step wall time": BASELINE.json configs[0] in full
+    # (N = 1024 to t = 1) and the first 1/16 time unit of configs[1] (N = 65 536), device-driven loop
+    block_step = None
+    if rank == 0 and args.workload == "step" and not args.no_block_step:
+        block_step = block_step_wall_time(nb, dev)
+
     if rank == 0:
         achieved = FLOPS_PER_PAIR * pairs_per_step / (kern_ms * 1e-3) / 1e12
         line = {
@@ -336,11 +343,35 @@ def run_ours(args):
                          "dfma_probe_tflops": probe_tf, "flops_per_pair": FLOPS_PER_PAIR,
                          "pipe_ceiling_frac": 85.0 / 106.0},
             "sections_ms": sections, "clocks": clk, "gpu_launches": int(launches),
-            "e2e": e2e, "cpu_baseline": cpu, "diag": diag,
+            "e2e": e2e, "cpu_baseline": cpu, "block_step_wall_time": block_step, "diag": diag,
         }
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def block_step_wall_time(nb, dev):
+    """Wall time per block step of the Hermite loop (nb_run_until, device-driven) on the seeded inputs of
+    BASELINE.json configs[0] (whole run) and configs[1] (first dt_max = 1/16 time unit)."""
+    import torch
+    from workloads import CONFIGS, config_inputs
+    out = []
+    for cfg, t_end in ((1, 1.0), (2, 1.0 / 16)):
+        c = CONFIGS[cfg]
+        pos, vel, m, _ = config_inputs(cfg)
+        g = nb.NBody(dev(pos), dev(vel), dev(m), c["eps"], c["eta"], dt_min=c["dt_min"], dt_max=c["dt_max"])
+        g.startup(); g.sync()
+        e0 = g.energy()
+        g.run_until(0.0)                       # builds the CUDA graph of this context outside the timed part
+        torch.cuda.synchronize()
+        t0 = time.perf_counter(); n = g.run_until(t_end); torch.cuda.synchronize(); wall = time.perf_counter() - t0
+        e1 = g.energy()
+        pairs = g.stats()["n_pairs"] - 2.0 * float(c["N"]) ** 2
+        out.append({"workload": "config%d_%s_to_t=%g" % (cfg, c["name"], t_end), "N": c["N"], "block_steps": int(n),
+                    "us_per_block_step": wall / max(n, 1) * 1e6, "wall_s": wall, "interactions_per_s": pairs / wall,
+                    "dE_over_E": float((e1[0] - e0[0]) / e0[0]), "loop": "device-driven CUDA-graph batches"})
+        g.close()
+    return out
 
 
 def main():
