@@ -9,7 +9,7 @@
 
 using namespace nb;
 
-static double __longlong_as_double_host(long long b)
+static double bits_to_double(long long b)
 {
     double d;
     memcpy(&d, &b, sizeof(d));
@@ -299,7 +299,7 @@ extern "C" int nb_run_steps(nb_ctx *ctx, int64_t n, double *log_t, int64_t *log_
         return set_err(ctx, NB_ESTATE, "nb_run_steps: a j-shard is set (nb_set_j_range)");
     if (ctx->use_graph && !log_t && !log_m && !log_ms) {
         if (n == 0) return NB_OK;
-        return graph_run(ctx, __longlong_as_double_host(0x7fefffffffffffffLL), n, nullptr);
+        return graph_run(ctx, bits_to_double(0x7fefffffffffffffLL), n, nullptr);
     }
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (log_ms) {
