@@ -145,7 +145,15 @@ def cpu_oracle_sample(pos, vel, accp, m, seconds_target=12.0):
     n_rows = max(T, (n_rows // T) * T)
     rows = rng.choice(N, size=n_rows, replace=False).astype(np.int32)
     t0 = time.perf_counter(); orc.force(pos, vel, accp, m, EPS, rows); t1 = time.perf_counter()
-    return dict(value=n_rows * N / (t1 - t0), unit=UNIT, cores=T, kind="oracle",
+    # the same on ONE core, on 1/8 of the rows (all cores and one core)
+    one = None
+    if T > 1:
+        r1 = rows[:max(1, n_rows // 8)]
+        orc.set_num_threads(1)
+        s0 = time.perf_counter(); orc.force(pos, vel, accp, m, EPS, r1); s1 = time.perf_counter()
+        orc.set_num_threads(T)
+        one = r1.size * N / (s1 - s0)
+    return dict(value=n_rows * N / (t1 - t0), unit=UNIT, cores=T, kind="oracle", value_one_core=one,
                 sample="orc_force (long-double direct summation, a3 only: a1/a2/a5/a6 are O(N), <0.1%% of a step): "
                        "%d i-rows x %d j in %.1f s" % (n_rows, N, t1 - t0)), n_rows, (t1 - t0)
 
