@@ -120,3 +120,29 @@ def test_sharded_world1_equals_plain_context(nb):
     nb.nb_get_full_state(a.g.ctx, xa); nb.nb_get_full_state(b.ctx, xb); a.g.sync(); b.sync()
     assert np.array_equal(host(xa), host(xb))
     a.close(); b.close()
+
+
+def test_sharded_driver_over_nccl_single_rank(nb):
+    """The default exchange of ShardedNBody (torch.distributed.all_reduce on the NCCL backend) with a
+    one-rank process group on this GPU: same states as the plain context, bit for bit."""
+    import socket
+    import torch.distributed as dist
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    dist.init_process_group("nccl", init_method="tcp://127.0.0.1:%d" % port, rank=0, world_size=1)
+    try:
+        n = 900
+        pos, vel, m = plummer(n, seed=45)
+        kw = dict(dt_min=2.0 ** -25, dt_max=2.0 ** -4)
+        a = ShardedNBody(dev(pos), dev(vel), dev(m), 1e-3, 0.45, **kw)       # rank/world from the process group
+        assert (a.rank, a.world, a.j_begin, a.j_end) == (0, 1, 0, n)
+        a.startup()
+        na = a.run_until(0.03125)
+        b = nb.NBody(dev(pos), dev(vel), dev(m), 1e-3, 0.45, **kw)
+        nb.nb_set_loop_mode(b.ctx, 0)
+        assert b.run_until(0.03125) == na and na > 10
+        xa = torch.empty((n, 21), dtype=torch.float64, device="cuda"); xb = torch.empty_like(xa)
+        nb.nb_get_full_state(a.g.ctx, xa); nb.nb_get_full_state(b.ctx, xb); a.g.sync(); b.sync()
+        assert np.array_equal(host(xa), host(xb))
+        a.close(); b.close()
+    finally:
+        dist.destroy_process_group()
