@@ -27,9 +27,11 @@
  * or reordering: loops run in index order; OpenMP only distributes independent i.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md section "Oracle pins".
- * Unpinned by the paper (free choices of this build, listed in DESIGN.md):
- *   the initial time-step rule and eta_init ("parity unpinned"),
- *   whole-trajectory values of config 1 ("parity unpinned": oracle <-> GPU only).
+ * Free choices of this build where the paper is silent (listed in DESIGN.md): the CHOICE of the
+ * initial time-step rule and of eta_init (G8) -- the arithmetic of the stated rule is pinned by
+ * hand-computed cases (tests/test_oracle_integrator.py::test_initial_dt_hand_cases); the
+ * whole-trajectory values of config 1 are compared oracle <-> GPU only ("parity unpinned by the
+ * paper": it prints no trajectory).
  */
 #include <math.h>
 #include <stdint.h>
@@ -241,7 +243,7 @@ double orc_timestep(const double *a, const double *j, const double *s, const dou
     return dt;
 }
 
-/* Start-up step (paper silent; reading G8, "parity unpinned"):
+/* Start-up step (paper silent; reading G8; pinned by hand-computed cases):
  * dt = pow2floor(eta_init * min(|a|/|jerk|, sqrt(|a|/|snap|))), clamped.         */
 double orc_initial_dt(const double *a, const double *j, const double *s, double eta_init,
                       double dt_min, double dt_max)

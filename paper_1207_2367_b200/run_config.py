@@ -219,6 +219,7 @@ def main():
                     help="the 'next' rows of SURVEY.md 8(f): split-j on/off sweep, heavy-particle run, Fig. 1 in FP64")
     ap.add_argument("--etas", default="0.3,0.45,0.6,0.8,1.0")
     ap.add_argument("--ns", default=None, help="comma-separated N list for --experiment fig1")
+    ap.add_argument("--ms", default=None, help="comma-separated active-set sizes for --config 4 (default: the config's five)")
     ap.add_argument("--heavy-frac", type=float, default=0.05)
     ap.add_argument("--loop", type=int, default=None, choices=[0, 1, 2], help="0: host-driven loop, 1: device-driven graph batches (default), 2: the same with programmatic dependent launch")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"],
@@ -255,7 +256,8 @@ def main():
         out = run_force(nb, 3, c, Ns, None)
     else:
         N = a.n or c["N"]
-        out = run_force(nb, 4, c, [N], [mm for mm in c["m"] if mm <= N])
+        ms = [int(x) for x in a.ms.split(",")] if a.ms else c["m"]
+        out = run_force(nb, 4, c, [N], [mm for mm in ms if mm <= N])
     out["precision"] = a.precision
     print(json.dumps(out), flush=True)
 

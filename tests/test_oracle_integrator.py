@@ -101,6 +101,61 @@ def test_timestep_uses_eq16_norm_combination(oracle):
     assert oracle.timestep(z, jerk, z, z, c4, z, 1.0, 2.0 ** -4, 1.0, 2.0 ** -25, 2.0 ** -3) == 2.0 ** -4
 
 
+# ---------------------------------------------------------------- start-up step (S0, reading G8)
+def test_initial_dt_hand_cases(oracle):
+    # S0 of SURVEY.md section 8(c): dt = pow2floor(eta_init * min(|a|/|jerk|, sqrt(|a|/|snap|))), clamped;
+    # a zero denominator drops its term, both zero -> dt_max.  The paper is silent on the rule (G8), but
+    # the arithmetic of the stated rule has hand-computable cases: every expected value below is a power
+    # of two worked out by hand, with eta_init itself a power of two so that the products are exact.
+    lo, hi = 2.0 ** -25, 2.0 ** -3
+    ex, ey, ez = np.array([1.0, 0, 0]), np.array([0, 1.0, 0]), np.array([0, 0, 1.0])
+    z = np.zeros(3)
+    f = lambda a, j, s, eta=0.25, lo=lo, hi=hi: oracle.initial_dt(a, j, s, eta, lo, hi)
+    big = 2.0 ** -40 * ez        # a tiny snap: sqrt(|a|/|snap|) = 2^20, never the minimum
+    # jerk term: |a|/|jerk| = 2^-3 exactly -> 0.25 * 2^-3 = 2^-5 stays 2^-5 (floor keeps an exact power)
+    assert f(ex, 8.0 * ey, big) == 2.0 ** -5
+    assert f(ex, 8.0 * (1 + 2 ** -52) * ey, big) == 2.0 ** -6      # just below 2^-5 -> 2^-6
+    assert f((1 + 2 ** -52) * ex, 8.0 * ey, big) == 2.0 ** -5      # just above stays 2^-5
+    assert f(1.75 * ex, 8.0 * ey, big) == 2.0 ** -5                # mantissa 1.75: floor, not round (-> 2^-4 if rounded)
+    # snap term wins and enters through a SQUARE ROOT: |a|/|snap| = 2^-10 -> sqrt = 2^-5 -> dt = 2^-7
+    # (without the sqrt: 0.25 * 2^-10 = 2^-12; with max instead of min: 0.25 * 1 = 2^-2 -> clamp 2^-3)
+    assert f(ex, ey, 2.0 ** 10 * ez) == 2.0 ** -7
+    # jerk term wins over the snap term (min, not max; not the snap term alone):
+    # |a|/|jerk| = 2^-6, sqrt(|a|/|snap|) = 2^-2 -> dt = 0.25 * 2^-6 = 2^-8
+    assert f(ex, 64.0 * ey, 16.0 * ez) == 2.0 ** -8
+    # the ratio is |a|/|jerk| (not its inverse): |a| = 2^-4, |jerk| = 1 -> 2^-4 -> dt = 2^-6
+    assert f(2.0 ** -4 * ex, ey, big) == 2.0 ** -6
+    # Euclidean norms of all three components: |a| = |(3,4,12)| = 13, |jerk| = |(0,5,12)|*8 = 104 -> 1/8
+    assert f(np.array([3.0, 4.0, 12.0]), 8.0 * np.array([0.0, 5.0, 12.0]), big) == 2.0 ** -5
+    # eta_init multiplies the ratio: halving it shifts exactly one level
+    assert f(ex, 8.0 * ey, big, eta=0.125) == 2.0 ** -6
+    # a zero denominator drops that term
+    assert f(ex, z, 2.0 ** 10 * ez) == 2.0 ** -7                    # jerk = 0: snap term alone
+    assert f(ex, 8.0 * ey, z) == 2.0 ** -5                          # snap = 0: jerk term alone
+    assert f(ex, z, z) == hi                                        # both zero -> dt_max
+    assert f(z, z, z) == hi                                         # a particle that feels nothing: dt_max, no 0/0
+    # clamps
+    assert f(ex, 2.0 ** -10 * ey, big) == hi                        # 0.25 * 2^10 -> clamp at dt_max
+    assert f(ex, 2.0 ** 40 * ey, big) == lo                         # 0.25 * 2^-40 -> clamp at dt_min
+    assert f(ex, 8.0 * ey, big, lo=2.0 ** -4, hi=2.0 ** -4) == 2.0 ** -4
+    # |a| = 0 with a non-zero jerk: the candidate is 0 -> dt_min (no NaN, no log of 0)
+    assert f(z, ey, ez) == lo
+
+
+def test_startup_uses_the_initial_dt_rule_per_particle(oracle):
+    # orc_startup assigns dt_i = initial_dt(a_i, jerk_i, snap_i): recompute every particle's step in numpy
+    # (plain double: norms, ratio, sqrt, min, floor to a power of two by frexp) from the committed a, jerk, snap.
+    pos, vel, m = plummer(96, seed=11)
+    eta_init, lo, hi = 0.01, 2.0 ** -25, 2.0 ** -4
+    it = oracle.Integrator(pos, vel, m, eps=1e-2, eta=0.45, dt_min=lo, dt_max=hi, eta_init=eta_init)
+    na, nj, ns = (np.sqrt((x * x).sum(axis=1)) for x in (it.acc, it.jerk, it.snap))
+    x = eta_init * np.minimum(na / nj, np.sqrt(na / ns))
+    mant, ex = np.frexp(x)                         # x = mant * 2^ex, mant in [0.5, 1)
+    want = np.clip(np.ldexp(0.5, ex), lo, hi)      # largest power of two <= x
+    assert np.array_equal(it.dt, want)
+    assert len(np.unique(it.dt)) > 2               # the case spans several levels
+
+
 # ---------------------------------------------------------------- Kepler orbit (closed form)
 def _kepler_rel(t, ecc):
     # start at apocentre on +x, a = 1, M = 1: mean anomaly pi + t; pericentre along -x
