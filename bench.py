@@ -4,8 +4,9 @@
 Workload (default): BASELINE.json configs[2] at N = 2^20 -- Plummer sphere, equal masses,
 eps = 1e-3, every particle active -- run as a COMPLETE Hermite block step, i.e. one pass of all
 hot-path rows: next block / gather (a1), predictor for all N (a2), evaluation of acc+jerk+snap
-of all N against all N (a3; a4 is the identity at one j-split), corrector (a5) and new time
-steps (a6).  All particles share one time level (dt_min = dt_max), so each step is exactly one
+of all N against all N (a3) in as many j-splits as keep the streamed piece L2-resident, summed in
+fixed order (a4; the launch geometry is read back from the library and printed in
+roofline.launch), corrector (a5) and new time steps (a6).  All particles share one time level (dt_min = dt_max), so each step is exactly one
 full-N evaluation: N^2 = 1.0995e12 pair interactions.  north_star quotes the metric (FP64 pair
 interactions/s, Tflop/s vs FP64 peak) on this full-N evaluation at N >= 1M.
 
@@ -32,9 +33,10 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# dram__bytes_read.sum + dram__bytes_write.sum of the evaluation kernel per launch, from the ncu capture
-# in profiles/r1_k_force_ncu_full_N2p20.md (bench.py cannot run under ncu itself); keyed by N
-NCU_DRAM_BYTES_PER_LAUNCH = {1 << 20: 384024320 + 450180352}
+# roofline.traffic comes from an ncu capture (bench.py cannot run under ncu itself): the JSON beside the
+# ncu summary records which library version and launch geometry it was taken on, and the figure is
+# reported only when both match what this run launched.
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "k_force_traffic.json")
 FLOPS_PER_PAIR = 85.0        # 32 DFMA x 2 + 11 DMUL + 10 DADD, counted in the SASS
 FLOPS_PER_PAIR_PAPER = 97.0  # the paper's convention (Table 2)
 # FP64 ALU peak derived from unit counts and clocks: 148 SMs x 64 FP64
@@ -44,6 +46,22 @@ METRIC = "fp64_pair_interactions_per_s"
 UNIT = "interactions/s"
 EPS = 1e-3
 DT_SHARED = 2.0 ** -10
+
+
+def ncu_traffic(N, launch, version):
+    """(bytes per launch or None, note): dram__bytes_read.sum + dram__bytes_write.sum of the evaluation kernel
+    from the committed ncu capture, valid only for the same library version, N and launch geometry."""
+    try:
+        with open(TRAFFIC_JSON) as f:
+            rec = json.load(f)
+    except Exception as e:
+        return None, "no capture record (%s)" % e
+    for c in rec.get("captures", []):
+        if c.get("N") == N and c.get("nb_version") == version and c.get("launch") == launch:
+            return int(c["dram_bytes_read"] + c["dram_bytes_write"]), \
+                "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum of the ncu --set full capture in %s" % c.get("source")
+    return None, "the committed ncu capture (%s) is of another library version / launch geometry than this run's (%s, %s)" % (
+        os.path.relpath(TRAFFIC_JSON, ROOT), version, launch)
 
 
 def parse():
@@ -153,7 +171,15 @@ def cpu_oracle_sample(pos, vel, accp, m, seconds_target=12.0):
         s0 = time.perf_counter(); orc.force(pos, vel, accp, m, EPS, r1); s1 = time.perf_counter()
         orc.set_num_threads(T)
         one = r1.size * N / (s1 - s0)
+    # the same source built with double arithmetic, -O3 -march=native (4x the rows: it is ~10x faster)
+    plain = None
+    try:
+        rows4 = rng.choice(N, size=min(N, 4 * n_rows), replace=False).astype(np.int32)
+        plain, _ = orc.force_plain_double_rate(pos, vel, accp, m, EPS, rows4)
+    except Exception:
+        plain = None
     return dict(value=n_rows * N / (t1 - t0), unit=UNIT, cores=T, kind="oracle", value_one_core=one,
+                value_plain_double_O3_native=plain,
                 sample="orc_force (long-double direct summation, a3 only: a1/a2/a5/a6 are O(N), <0.1%% of a step): "
                        "%d i-rows x %d j in %.1f s" % (n_rows, N, t1 - t0)), n_rows, (t1 - t0)
 
@@ -276,6 +302,7 @@ def run_ours(args):
     clk = clocks.stop() if rank == 0 else None
     ms_total = t_start.elapsed_time(t_end)
     launches = nb.nb_get_stats(ctx)["n_launch"] - launches0
+    launch = {k: int(v) for k, v in nb.nb_get_launch(ctx).items()}   # what the last evaluation launched
     kern_ms = float(np.mean([a.elapsed_time(b) for a, b in force_ms])) if force_ms else float("nan")
     sections = {k: float(np.mean([a.elapsed_time(b) for a, b in v])) for k, v in sect.items() if v}
     ms_total = max_over_ranks(ms_total, world)
@@ -331,6 +358,10 @@ def run_ours(args):
 
     if rank == 0:
         achieved = FLOPS_PER_PAIR * pairs_per_step / (kern_ms * 1e-3) / 1e12
+        traffic, traffic_note = ncu_traffic(N, launch, nb.nb_version())
+        kname = "k_force<%d,%d> variant %s, FP64, %d j-lane(s) per i" % (
+            launch["threads"], launch["tile"], "A" if launch["threads"] == 128 else "B", launch["jlanes"])
+        algorithmic = 80.0 * N * 2 + 72.0 * N * (launch["splits"] if launch["splits"] > 1 else 1)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -341,11 +372,15 @@ def run_ours(args):
                        "l2": "flushed between steps (256 MiB memset inside the timed region); state 176 MB + stream 84 MB"},
             "tflops_85": value * FLOPS_PER_PAIR / 1e12, "tflops_97_paper_convention": value * FLOPS_PER_PAIR_PAPER / 1e12,
             "fp64_peak_frac_85": value / world * FLOPS_PER_PAIR / 1e12 / FP64_PEAK_TFLOPS,
-            "roofline": {"bound": "alu", "kernel": "k_force<128,128,4,1>", "achieved": achieved,
+            "roofline": {"bound": "alu", "kernel": kname, "achieved": achieved,
                          "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
-                         "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(N), "traffic_unit": "bytes per launch (dram__bytes_read.sum + "
-                         "dram__bytes_write.sum of the ncu --set full capture in profiles/r1_k_force_ncu_full_N2p20.md); algorithmic 4.70e8",
-                         "kernel_ms": kern_ms, "launch": "grid 8192 x 4 splits, 128 threads; + k_reduce_thread" if N == 1 << 20 else None,
+                         "frac_vs_probe": (achieved / probe_tf) if probe_tf else None,
+                         "traffic": traffic, "traffic_note": traffic_note,
+                         "algorithmic_bytes": algorithmic,
+                         "kernel_ms": kern_ms,
+                         "launch": dict(launch, grid=[launch["ctas"] // max(launch["splits"], 1), launch["splits"]],
+                                        reduction="fixed-order sum of the split partials" if launch["splits"] > 1 else "none (one split)",
+                                        version=nb.nb_version()),
                          "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md section 7); "
                                         "MEASURED_PEAKS.json has no FP64 entry",
                          "dfma_probe_tflops": probe_tf, "flops_per_pair": FLOPS_PER_PAIR,

@@ -58,7 +58,12 @@ enum {
  *   the legacy default stream) on which every later call of this context enqueues.
  * After nb_init: t_i = 0, all derivatives 0, the predicted arrays hold (pos, vel, a_pred = 0)
  * so nb_force may be called at once (force-only use); time-step limits are the paper's
- * 2^-25 and 2^-3, eta_init = 0.01 (G8).  *ctx is NULL on failure.          */
+ * 2^-25 and 2^-3, eta_init = 0.01 (G8).  *ctx is NULL on failure.
+ * nb_init does NOT run the start-up S0 (SURVEY.md section 8(b) sketched it inside nb_init): S0 is
+ * nb_startup, because it costs two full-N evaluations (2 N^2 pairs: 6 s at N = 2^20, 6 min at 2^23)
+ * that force-only use (configs 3, 4) and a context that loads a checkpoint (nb_set_full_state) must
+ * not pay, and because nb_set_limits / nb_set_precision must be able to act before it.
+ * nb_run_until / nb_run_steps run it implicitly when it has not run.                        */
 int nb_init(nb_ctx **ctx, int64_t N, const double *pos, const double *vel, const double *mass,
             double eps, double eta, void *cuda_stream);
 
@@ -68,7 +73,9 @@ int nb_set_limits(nb_ctx *ctx, double dt_min, double dt_max, double eta_init);
 
 /* Start-up S0 (paper silent; G8): pass 1 evaluates a, jerk with a_pred = 0, pass 2 evaluates
  * a, jerk, snap with a_pred = a; crackle = 0; dt_i = pow2floor(eta_init * min(|a|/|jerk|,
- * sqrt(|a|/|snap|))) clamped to the limits.  Two full-N evaluations (2 N^2 pairs).          */
+ * sqrt(|a|/|snap|))) clamped to the limits.  Two full-N evaluations (2 N^2 pairs).
+ * NB_ESTATE when a proper j-slice is set (nb_set_j_range): a sliced start-up needs the exchange
+ * between its passes and is driven call by call with nb_startup_commit.                      */
 int nb_startup(nb_ctx *ctx);
 
 /* The two commits of nb_startup as separate calls, for callers that must exchange the evaluated
@@ -96,7 +103,12 @@ int nb_predict(nb_ctx *ctx, double t);
  *       NULL otherwise           -> the scheduler's set (n_active must equal its size).
  *   acc, jerk, snap [dev|host] [n_active][3], each may be NULL (not returned).
  * The evaluated values are also kept inside the context for nb_correct_and_step.
- * Needs valid predicted data: after nb_init, nb_set_pred, nb_predict or nb_startup.         */
+ * Needs valid predicted data: after nb_init, nb_set_pred, nb_predict or nb_startup.
+ * The indices are NOT range-checked on the hot path (an index outside [0, N) reads outside the
+ * predicted stream); nb_set_debug(ctx, 1) adds a device-side check that makes the call return
+ * NB_EINVAL, naming the first offending slot, before anything is evaluated.
+ * With a proper j-slice set (nb_set_j_range) the values are slice partials: nb_correct_and_step
+ * refuses them until nb_set_forces has stored the reduced buffer.                            */
 int nb_force(nb_ctx *ctx, const int32_t *active_idx, int64_t n_active, double *acc,
              double *jerk, double *snap);
 
@@ -122,7 +134,10 @@ int nb_run_steps(nb_ctx *ctx, int64_t n, double *log_t, int64_t *log_m, float *l
 
 /* Diagnostics at the current time (Eq. 2; Eq. 20):
  * out [host] = {E, K, W, Px, Py, Pz, Lx, Ly, Lz}; W = -sum_{i<j} m_i m_j/sqrt(r_ij^2+eps^2).
- * Particles not at the current time are predicted to it first (Eq. 3-7).                    */
+ * Particles not at the current time are predicted to it first (Eq. 3-7), into a scratch buffer:
+ * the predicted arrays that nb_force reads (nb_predict, nb_set_pred, nb_set_pred_acc) are left
+ * untouched.  With eps = 0 two DISTINCT particles at the same position are outside the domain
+ * (G12); such a pair contributes nothing instead of an infinite W.                           */
 int nb_energy(nb_ctx *ctx, double out[9]);
 
 /* Copy out the committed state; any pointer may be NULL.  pos, vel [dev|host] [N][3];
@@ -184,12 +199,20 @@ int nb_set_forces(nb_ctx *ctx, const double *buf);
  * ~1e-16; everything else (predictor, corrector, time steps, energy) stays binary64.        */
 int nb_set_precision(nb_ctx *ctx, int mode);
 
-/* Driver of nb_run_until / nb_run_steps: 1 (default) = device-driven CUDA-graph batches,
- * 2 = the same graph with its kernels chained by programmatic dependent launch (each kernel is
- * launched while its predecessor still runs and waits on the device for its completion; measured
- * slower than plain graph edges on B200, kept for comparison), 0 = the host issues nb_next_block /
- * nb_predict / nb_force / nb_correct_and_step per step.  All give bit-identical states.
- * nb_run_steps with a per-step log always uses 0.                                           */
+/* Debug switch (Errors): 1 = nb_force range-checks a caller-supplied
+ * active_idx on the device (one extra small kernel and a stream synchronisation per call) and
+ * returns NB_EINVAL instead of reading out of bounds; 0 (default) = no check, no cost.       */
+int nb_set_debug(nb_ctx *ctx, int on);
+
+/* Driver of nb_run_until / nb_run_steps (all give bit-identical states):
+ *   0  the host issues nb_next_block / nb_predict / nb_force / nb_correct_and_step per step;
+ *   1  device-driven CUDA-graph batches (kernels read (t_next, n_active) from device memory);
+ *   2  the same graph with its kernels chained by programmatic dependent launch (measured slower than
+ *      plain graph edges on B200, kept for comparison);
+ *   3  ONE kernel resident on one thread-block cluster runs every step, its phases separated by the
+ *      hardware cluster barrier instead of kernel boundaries (no host round trip and no launch per step;
+ *      the small blocks); at most 16 SMs work, so it serves N <= 16384 (NB_EINVAL above).
+ * Default: 3 for N <= 2048, else 1.  nb_run_steps with a per-step log always uses 0.          */
 int nb_set_loop_mode(nb_ctx *ctx, int device_driven);
 
 /* What the last nb_force launched: out [host] = {threads per CTA, j-lanes per i, j-splits,
@@ -201,22 +224,10 @@ int nb_get_launch(nb_ctx *ctx, int64_t out[5]);
  * It is the measured denominator quoted beside the nominal FP64 peak. */
 int nb_probe_fp64_peak(nb_ctx *ctx, int64_t iters, double *flops, float *ms);
 
-/* Operand-fetch probe of the FP64 datapath: streams of independent
- * DFMAs whose source operands are, per mode,
- *   0: one register + two immediates (pure pipe rate)      1: three distinct registers
- *   2: three registers, one shared by groups of three consecutive DFMAs (reuse cache)
- *   3: two distinct registers (a*a + c)
- *   4: three registers, the first shared by ALL DFMAs (reuse-cache hit on every instruction but
- *      the one after each scheduler yield)
- *   5: alternating 3-register DFMA and a DADD that shares one source with it (1 fresh read)
- * *cycles_per_inst [host] = SM-clock cycles per warp instruction per SM sub-partition, at the
- * clock `sm_mhz` the caller passes (e.g. the nvidia-smi reading).                          */
-int nb_probe_fp64_operands(nb_ctx *ctx, int mode, int64_t iters, double sm_mhz, double *cycles_per_inst);
-
 const char *nb_last_error(const nb_ctx *ctx);
 void nb_free(nb_ctx *ctx);
 
-/* Library version string, e.g. "nb-b200 0.1 (sm_100a)".                                     */
+/* Library version string, e.g. "nb-b200 0.2 (sm_100a)".                                     */
 const char *nb_version(void);
 
 #ifdef __cplusplus

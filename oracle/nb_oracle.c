@@ -41,7 +41,14 @@
 #include <omp.h>
 #endif
 
-typedef long double ld;
+/* The arithmetic type.  The oracle IS the long-double build (the default).  bench.py also times a second
+ * build of this same file with -DORC_REAL=double -DORC_SQRT=sqrt -O3 -march=native, as a plain-double CPU
+ * baseline for the throughput table only; no test compares against that build.                       */
+#ifndef ORC_REAL
+#define ORC_REAL long double
+#define ORC_SQRT sqrtl
+#endif
+typedef ORC_REAL ld;
 
 int orc_num_threads(void) {
 #ifdef _OPENMP
@@ -81,7 +88,7 @@ void orc_force(int64_t N, const double *rp, const double *vp, const double *ap,
                 a[d] = (ld)ap[3 * j + d] - (ld)ap[3 * i + d];
             }
             const ld s = r[0] * r[0] + r[1] * r[1] + r[2] * r[2] + eps2; /* r_ij^2 (+eps^2) */
-            const ld r3 = s * sqrtl(s);                                  /* r_ij^3          */
+            const ld r3 = s * ORC_SQRT(s);                                  /* r_ij^3          */
             const ld rv = r[0] * v[0] + r[1] * v[1] + r[2] * v[2];
             const ld vv = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
             const ld ra = r[0] * a[0] + r[1] * a[1] + r[2] * a[2];
@@ -294,7 +301,7 @@ void orc_energy(int64_t N, const double *r, const double *v, const double *mass,
                 const ld dx = (ld)r[3 * j] - (ld)r[3 * i];
                 const ld dy = (ld)r[3 * j + 1] - (ld)r[3 * i + 1];
                 const ld dz = (ld)r[3 * j + 2] - (ld)r[3 * i + 2];
-                wi += (ld)mass[j] / sqrtl(dx * dx + dy * dy + dz * dz + eps2);
+                wi += (ld)mass[j] / ORC_SQRT(dx * dx + dy * dy + dz * dz + eps2);
             }
             Wloc -= (ld)mass[i] * wi;
         }

@@ -33,6 +33,31 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
+def build_plain_double(force: bool = False) -> str:
+    """The same source with the arithmetic type set to double and -O3 -march=native: bench.py's
+    plain-double CPU throughput baseline (never used as a correctness reference)."""
+    out = os.path.join(_HERE, "libnb_oracle_f64.so")
+    if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-std=c11", "-O3", "-march=native", "-fopenmp", "-ffp-contract=off", "-DORC_REAL=double",
+               "-DORC_SQRT=sqrt", "-fPIC", "-shared", "-o", out, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return out
+
+
+def force_plain_double_rate(pos_pred, vel_pred, acc_pred, mass, eps, idx):
+    """Pairs/s of orc_force in the plain-double build on the rows idx (timing aid for bench.py)."""
+    import time
+    L = C.CDLL(build_plain_double())
+    L.orc_force.argtypes = [C.c_int64, _dp, _dp, _dp, _dp, C.c_double, _ip, C.c_int64, _dp, _dp, _dp]
+    rp, vp, ap, m = _arr(pos_pred), _arr(vel_pred), _arr(acc_pred), _arr(mass)
+    idx = np.ascontiguousarray(idx, dtype=np.int32)
+    n = idx.shape[0]
+    acc = np.zeros((n, 3)); jerk = np.zeros((n, 3)); snap = np.zeros((n, 3))
+    t0 = time.perf_counter()
+    L.orc_force(m.shape[0], _d(rp), _d(vp), _d(ap), _d(m), float(eps), idx.ctypes.data_as(_ip), n, _d(acc), _d(jerk), _d(snap))
+    return n * m.shape[0] / (time.perf_counter() - t0), acc
+
+
 def _d(x):
     return x.ctypes.data_as(_dp)
 

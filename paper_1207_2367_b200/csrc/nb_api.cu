@@ -44,10 +44,11 @@ static void release(nb_ctx *ctx)
     for (void *b : bufs)
         if (b) cudaFree(b);
     if (ctx->h_sched) cudaFreeHost(ctx->h_sched);
+    if (ctx->h_dbg) cudaFreeHost(ctx->h_dbg);
     delete ctx;
 }
 
-extern "C" const char *nb_version(void) { return "nb-b200 0.1 (sm_100a)"; }
+extern "C" const char *nb_version(void) { return "nb-b200 0.2 (sm_100a)"; }
 
 extern "C" const char *nb_last_error(const nb_ctx *ctx) { return ctx ? ctx->err : "null context"; }
 
@@ -70,6 +71,20 @@ static int copy_out(nb_ctx *ctx, void *dst, const void *src_dev, size_t bytes)
     NB_CUDA(ctx, cudaMemcpyAsync(dst, src_dev, bytes, cudaMemcpyDefault, ctx->stream));
     return NB_OK;
 }
+
+// The staging buffer grows on demand: [n][3] copies need 9 n doubles, nb_get_derivs 12 Npad, a
+// checkpoint 21 Npad.  Growing synchronises the stream (pending copies still use the old buffer).
+int nb::reserve_stage(nb_ctx *ctx, size_t doubles)
+{
+    if (doubles <= ctx->stage_cap) return NB_OK;
+    if (ctx->stage) { NB_CUDA(ctx, cudaStreamSynchronize(ctx->stream)); cudaFree(ctx->stage); }
+    ctx->stage = nullptr; ctx->stage_cap = 0;
+    NB_CUDA(ctx, cudaMalloc((void **)&ctx->stage, doubles * sizeof(double)));
+    ctx->stage_cap = doubles;
+    return NB_OK;
+}
+
+static bool sliced(const nb_ctx *ctx) { return ctx->j_begin != 0 || ctx->j_end != ctx->N; }
 
 extern "C" int nb_init(nb_ctx **out, int64_t N, const double *pos, const double *vel, const double *mass,
                        double eps, double eta, void *cuda_stream)
@@ -109,7 +124,7 @@ extern "C" int nb_init(nb_ctx **out, int64_t N, const double *pos, const double 
         (rc = dev_alloc(ctx, &ctx->s, 3 * P)) || (rc = dev_alloc(ctx, &ctx->c, 3 * P)) ||
         (rc = dev_alloc(ctx, &ctx->jp, REC * P)) || (rc = dev_alloc(ctx, &ctx->active, P)) ||
         (rc = dev_alloc(ctx, &ctx->user_idx, P)) || (rc = dev_alloc(ctx, &ctx->f1, 9 * P)) ||
-        (rc = dev_alloc(ctx, &ctx->stage, 21 * P)) || (rc = dev_alloc(ctx, &ctx->d_tmin, 2)))
+        (rc = reserve_stage(ctx, 12 * P)) || (rc = dev_alloc(ctx, &ctx->d_tmin, 2)))
         return fail(rc);
     ctx->n_sched_blocks = (N + 2047) / 2048;
     if ((rc = dev_alloc(ctx, &ctx->blk_count, (size_t)ctx->n_sched_blocks + 1)) ||
@@ -118,11 +133,13 @@ extern "C" int nb_init(nb_ctx **out, int64_t N, const double *pos, const double 
     if (cudaHostAlloc((void **)&ctx->h_sched, sizeof(Sched), cudaHostAllocMapped) != cudaSuccess) return fail(NB_ENOMEM);
     if (cudaHostGetDevicePointer((void **)&ctx->d_sched, ctx->h_sched, 0) != cudaSuccess) return fail(NB_ECUDA);
     ctx->h_sched->t_next = 0.0; ctx->h_sched->n_active = 0;
+    if (cudaHostAlloc((void **)&ctx->h_dbg, 2 * sizeof(int32_t), cudaHostAllocMapped) != cudaSuccess) return fail(NB_ENOMEM);
+    if (cudaHostGetDevicePointer((void **)&ctx->d_dbg, ctx->h_dbg, 0) != cudaSuccess) return fail(NB_ECUDA);
     if ((rc = dev_alloc(ctx, &ctx->ctl, 1)) || (rc = dev_alloc(ctx, &ctx->geom_cache, (size_t)GEOM_CACHE_M + 1)))
         return fail(rc);
     if (cudaHostAlloc((void **)&ctx->h_ctl, sizeof(StepCtl), cudaHostAllocDefault) != cudaSuccess) return fail(NB_ENOMEM);
     memset(ctx->h_ctl, 0, sizeof(StepCtl));
-    ctx->use_graph = 1;
+    ctx->use_graph = N <= RES_AUTO_N ? 3 : 1;
     ctx->j_begin = 0; ctx->j_end = N;
     if ((rc = query_force_occupancy(ctx))) return fail(rc);
 
@@ -153,6 +170,9 @@ extern "C" int nb_startup(nb_ctx *ctx)
 {
     if (!ctx) return NB_EINVAL;
     if (ctx->started) return set_err(ctx, NB_ESTATE, "nb_startup: already started");
+    if (sliced(ctx))
+        return set_err(ctx, NB_ESTATE, "nb_startup: a j-slice is set (nb_set_j_range); drive the start-up call by call "
+                                       "(nb_force, exchange, nb_startup_commit)");
     // a context that steps will split small active sets over many j-pieces: take the partial-sum buffer
     // now (up to 0.5 GB at large N) rather than inside the first block step
     NB_TRY(reserve_partials(ctx, ctx->partials_limit));
@@ -163,7 +183,7 @@ extern "C" int nb_startup(nb_ctx *ctx)
     NB_TRY(launch_force(ctx, nullptr, ctx->N));      // pass 2: a, jerk, snap
     NB_TRY(launch_startup_commit(ctx, 2));           // commit, crackle = 0, initial dt
     ctx->started = true; ctx->pred_valid = true; ctx->t_pred = 0.0; ctx->t_now = 0.0;
-    ctx->have_block = false; ctx->evaluated = false;
+    ctx->have_block = false; ctx->evaluated = false; ctx->eval_partial = false;
     return NB_OK;
 }
 
@@ -176,7 +196,7 @@ extern "C" int nb_startup_commit(nb_ctx *ctx, int pass)
     NB_TRY(launch_startup_commit(ctx, pass));
     if (pass == 2) {
         ctx->started = true; ctx->pred_valid = true; ctx->t_pred = 0.0; ctx->t_now = 0.0;
-        ctx->have_block = false; ctx->evaluated = false;
+        ctx->have_block = false; ctx->evaluated = false; ctx->eval_partial = false;
     }
     return NB_OK;
 }
@@ -189,7 +209,7 @@ extern "C" int nb_next_block(nb_ctx *ctx, double *t_next, int64_t *n_active)
     NB_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     ctx->t_next = ctx->h_sched->t_next;
     ctx->n_active = (int64_t)ctx->h_sched->n_active;
-    ctx->have_block = true; ctx->evaluated = false;
+    ctx->have_block = true; ctx->evaluated = false; ctx->eval_partial = false;
     if (t_next) *t_next = ctx->t_next;
     if (n_active) *n_active = ctx->n_active;
     return NB_OK;
@@ -207,7 +227,7 @@ extern "C" int nb_predict(nb_ctx *ctx, double t)
     if (!ctx) return NB_EINVAL;
     if (!(t >= ctx->t_now) || !isfinite(t)) return set_err(ctx, NB_EINVAL, "nb_predict: t = %g is earlier than the current time %g", t, ctx->t_now);
     NB_TRY(launch_predict(ctx, t));
-    ctx->pred_valid = true; ctx->t_pred = t; ctx->evaluated = false;
+    ctx->pred_valid = true; ctx->t_pred = t; ctx->evaluated = false; ctx->eval_partial = false;
     return NB_OK;
 }
 
@@ -223,6 +243,12 @@ extern "C" int nb_force(nb_ctx *ctx, const int32_t *active_idx, int64_t n_active
     if (active_idx) {
         NB_TRY(copy_in(ctx, ctx->user_idx, active_idx, (size_t)n_active * sizeof(int32_t)));
         list = ctx->user_idx;
+        if (ctx->debug) {
+            NB_TRY(launch_check_indices(ctx, list, n_active));
+            if (ctx->h_dbg[0] > 0)
+                return set_err(ctx, NB_EINVAL, "nb_force: %d of the %lld entries of active_idx are outside [0, %lld); first at slot %d",
+                               (int)ctx->h_dbg[0], (long long)n_active, (long long)ctx->N, (int)ctx->h_dbg[1]);
+        }
     } else if (n_active == ctx->N) {
         list = nullptr;  // all particles, index order
         sched_set = ctx->have_block && ctx->n_active == ctx->N;
@@ -235,8 +261,12 @@ extern "C" int nb_force(nb_ctx *ctx, const int32_t *active_idx, int64_t n_active
     }
     NB_TRY(launch_force(ctx, list, n_active));
     ctx->n_eval = n_active;
-    ctx->evaluated = sched_set && ctx->t_pred == ctx->t_next;
+    // over a proper j-slice these are partial sums: the corrector must not run on them (nb_set_forces)
+    const bool block_eval = sched_set && ctx->t_pred == ctx->t_next;
+    ctx->evaluated = block_eval && !sliced(ctx);
+    ctx->eval_partial = block_eval && sliced(ctx);
     if ((acc || jerk || snap) && n_active > 0) {
+        NB_TRY(reserve_stage(ctx, 9 * (size_t)n_active));
         NB_TRY(launch_unpack_f1(ctx, n_active));
         const size_t bytes = 3 * (size_t)n_active * sizeof(double);
         if (acc) NB_TRY(copy_out(ctx, acc, ctx->stage, bytes));
@@ -249,12 +279,15 @@ extern "C" int nb_force(nb_ctx *ctx, const int32_t *active_idx, int64_t n_active
 extern "C" int nb_correct_and_step(nb_ctx *ctx)
 {
     if (!ctx) return NB_EINVAL;
+    if (ctx->have_block && ctx->eval_partial)
+        return set_err(ctx, NB_ESTATE, "nb_correct_and_step: the evaluated values are j-slice partials (nb_set_j_range); "
+                                       "all-reduce nb_get_forces and store the sums with nb_set_forces first");
     if (!ctx->have_block || !ctx->evaluated)
         return set_err(ctx, NB_ESTATE, "nb_correct_and_step: needs nb_next_block, nb_predict(t_next) and nb_force on the scheduler's set");
     const int64_t m = ctx->n_active;
     NB_TRY(launch_correct(ctx, m == ctx->N ? nullptr : ctx->active, m, ctx->t_next));
     ctx->t_now = ctx->t_next;
-    ctx->have_block = false; ctx->evaluated = false;
+    ctx->have_block = false; ctx->evaluated = false; ctx->eval_partial = false;
     ctx->n_steps += 1;
     int b = 0;
     while ((((int64_t)1) << (b + 1)) <= m) ++b;
@@ -275,9 +308,10 @@ extern "C" int nb_run_until(nb_ctx *ctx, double t_end, int64_t *n_steps)
 {
     if (!ctx) return NB_EINVAL;
     if (!isfinite(t_end)) return set_err(ctx, NB_EINVAL, "nb_run_until: bad t_end");
-    if (!ctx->started) NB_TRY(nb_startup(ctx));
-    if (ctx->j_begin != 0 || ctx->j_end != ctx->N)
+    if (sliced(ctx))   // before the implicit start-up: a refused call leaves the context untouched
         return set_err(ctx, NB_ESTATE, "nb_run_until: a j-shard is set (nb_set_j_range); drive the steps call by call and all-reduce nb_get_forces");
+    if (!ctx->started) NB_TRY(nb_startup(ctx));
+    if (ctx->use_graph == 3) return resident_run(ctx, t_end, INT64_MAX, n_steps);
     if (ctx->use_graph) return graph_run(ctx, t_end, INT64_MAX, n_steps);
     int64_t n = 0;
     for (;;) {
@@ -294,11 +328,11 @@ extern "C" int nb_run_until(nb_ctx *ctx, double t_end, int64_t *n_steps)
 extern "C" int nb_run_steps(nb_ctx *ctx, int64_t n, double *log_t, int64_t *log_m, float *log_ms)
 {
     if (!ctx || n < 0) return NB_EINVAL;
+    if (sliced(ctx)) return set_err(ctx, NB_ESTATE, "nb_run_steps: a j-shard is set (nb_set_j_range)");
     if (!ctx->started) NB_TRY(nb_startup(ctx));
-    if (ctx->j_begin != 0 || ctx->j_end != ctx->N)
-        return set_err(ctx, NB_ESTATE, "nb_run_steps: a j-shard is set (nb_set_j_range)");
     if (ctx->use_graph && !log_t && !log_m && !log_ms) {
         if (n == 0) return NB_OK;
+        if (ctx->use_graph == 3) return resident_run(ctx, bits_to_double(0x7fefffffffffffffLL), n, nullptr);
         return graph_run(ctx, bits_to_double(0x7fefffffffffffffLL), n, nullptr);
     }
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -333,17 +367,21 @@ extern "C" int nb_run_steps(nb_ctx *ctx, int64_t n, double *log_t, int64_t *log_
 extern "C" int nb_energy(nb_ctx *ctx, double out[9])
 {
     if (!ctx || !out) return NB_EINVAL;
-    // positions and velocities of every particle at the current time: the predictor is the
-    // identity for particles already there (h = 0)
-    NB_TRY(launch_predict(ctx, ctx->t_now));
-    ctx->pred_valid = true; ctx->t_pred = ctx->t_now; ctx->evaluated = false;
-    return launch_energy(ctx, out);
+    // positions and velocities of every particle at the current time (the predictor is the identity
+    // for particles already there, h = 0), written to a scratch copy of the record stream so that the
+    // predicted data nb_force reads stay what the caller last set or predicted
+    const size_t P = (size_t)ctx->Npad, N = (size_t)ctx->N;
+    NB_TRY(reserve_stage(ctx, REC * P));
+    NB_TRY(launch_predict(ctx, ctx->t_now, ctx->stage));
+    if (P > N) NB_CUDA(ctx, cudaMemsetAsync(ctx->stage + REC * N, 0, REC * (P - N) * sizeof(double), ctx->stream));
+    return launch_energy(ctx, ctx->stage, out);
 }
 
 extern "C" int nb_get_state(nb_ctx *ctx, double *pos, double *vel, double *t, double *dt)
 {
     if (!ctx) return NB_EINVAL;
     const size_t P = (size_t)ctx->Npad, N = (size_t)ctx->N;
+    NB_TRY(reserve_stage(ctx, 6 * P));
     if (pos) { NB_TRY(launch_pack3(ctx, ctx->r, ctx->stage)); NB_TRY(copy_out(ctx, pos, ctx->stage, 3 * N * sizeof(double))); }
     if (vel) { NB_TRY(launch_pack3(ctx, ctx->v, ctx->stage + 3 * P)); NB_TRY(copy_out(ctx, vel, ctx->stage + 3 * P, 3 * N * sizeof(double))); }
     if (t) NB_TRY(copy_out(ctx, t, ctx->t, N * sizeof(double)));
@@ -357,6 +395,7 @@ extern "C" int nb_get_derivs(nb_ctx *ctx, double *acc, double *jerk, double *sna
     const size_t P = (size_t)ctx->Npad, N = (size_t)ctx->N;
     double *dst[4] = {acc, jerk, snap, crackle};
     const double *src[4] = {ctx->a, ctx->j, ctx->s, ctx->c};
+    NB_TRY(reserve_stage(ctx, 12 * P));
     for (int q = 0; q < 4; ++q)
         if (dst[q]) {
             NB_TRY(launch_pack3(ctx, src[q], ctx->stage + 3 * P * q));
@@ -370,6 +409,7 @@ extern "C" int nb_get_pred(nb_ctx *ctx, double *pos, double *vel, double *acc)
     if (!ctx) return NB_EINVAL;
     if (!ctx->pred_valid) return set_err(ctx, NB_ESTATE, "nb_get_pred: no predicted data");
     const size_t P = (size_t)ctx->Npad, N = (size_t)ctx->N;
+    NB_TRY(reserve_stage(ctx, 9 * P));
     NB_TRY(launch_get_pred(ctx, ctx->stage, ctx->stage + 3 * P, ctx->stage + 6 * P));
     if (pos) NB_TRY(copy_out(ctx, pos, ctx->stage, 3 * N * sizeof(double)));
     if (vel) NB_TRY(copy_out(ctx, vel, ctx->stage + 3 * P, 3 * N * sizeof(double)));
@@ -381,9 +421,10 @@ extern "C" int nb_set_pred_acc(nb_ctx *ctx, const double *acc_pred)
 {
     if (!ctx || !acc_pred) return NB_EINVAL;
     if (!ctx->pred_valid) return set_err(ctx, NB_ESTATE, "nb_set_pred_acc: no predicted data");
+    NB_TRY(reserve_stage(ctx, 3 * (size_t)ctx->Npad));
     NB_TRY(copy_in(ctx, ctx->stage, acc_pred, 3 * (size_t)ctx->N * sizeof(double)));
     NB_TRY(launch_set_pred(ctx, nullptr, nullptr, ctx->stage, false, true));
-    ctx->evaluated = false;
+    ctx->evaluated = false; ctx->eval_partial = false;
     return NB_OK;
 }
 
@@ -391,17 +432,19 @@ extern "C" int nb_set_pred(nb_ctx *ctx, const double *pos, const double *vel, co
 {
     if (!ctx || !pos || !vel) return NB_EINVAL;
     const size_t P = (size_t)ctx->Npad, N = (size_t)ctx->N;
+    NB_TRY(reserve_stage(ctx, 9 * P));
     NB_TRY(copy_in(ctx, ctx->stage, pos, 3 * N * sizeof(double)));
     NB_TRY(copy_in(ctx, ctx->stage + 3 * P, vel, 3 * N * sizeof(double)));
     if (acc) NB_TRY(copy_in(ctx, ctx->stage + 6 * P, acc, 3 * N * sizeof(double)));
     NB_TRY(launch_set_pred(ctx, ctx->stage, ctx->stage + 3 * P, ctx->stage + 6 * P, true, acc != nullptr));
-    ctx->pred_valid = true; ctx->evaluated = false;
+    ctx->pred_valid = true; ctx->evaluated = false; ctx->eval_partial = false;
     return NB_OK;
 }
 
 extern "C" int nb_get_full_state(nb_ctx *ctx, double *state)
 {
     if (!ctx || !state) return NB_EINVAL;
+    NB_TRY(reserve_stage(ctx, 21 * (size_t)ctx->Npad));
     NB_TRY(launch_full_state(ctx, ctx->stage, false));
     return copy_out(ctx, state, ctx->stage, 21 * (size_t)ctx->N * sizeof(double));
 }
@@ -409,12 +452,13 @@ extern "C" int nb_get_full_state(nb_ctx *ctx, double *state)
 extern "C" int nb_set_full_state(nb_ctx *ctx, const double *state)
 {
     if (!ctx || !state) return NB_EINVAL;
+    NB_TRY(reserve_stage(ctx, 21 * (size_t)ctx->Npad));
     NB_TRY(copy_in(ctx, ctx->stage, state, 21 * (size_t)ctx->N * sizeof(double)));
     NB_TRY(launch_full_state(ctx, ctx->stage, true));
     NB_TRY(launch_tmax(ctx));
     NB_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     ctx->t_now = ctx->h_sched->t_next;
-    ctx->started = true; ctx->have_block = false; ctx->evaluated = false; ctx->pred_valid = false;
+    ctx->started = true; ctx->have_block = false; ctx->evaluated = false; ctx->eval_partial = false; ctx->pred_valid = false;
     return NB_OK;
 }
 
@@ -443,7 +487,7 @@ extern "C" int nb_set_j_range(nb_ctx *ctx, int64_t j_begin, int64_t j_end)
         (j_end != ctx->N && (j_end % TILE_ALIGN) != 0))
         return set_err(ctx, NB_EINVAL, "nb_set_j_range: need 0 <= j_begin < j_end <= N, both multiples of %d (j_end may be N)", TILE_ALIGN);
     ctx->j_begin = j_begin; ctx->j_end = j_end;
-    ctx->evaluated = false;
+    ctx->evaluated = false; ctx->eval_partial = false;
     return NB_OK;
 }
 
@@ -451,6 +495,7 @@ extern "C" int nb_get_forces(nb_ctx *ctx, double *buf)
 {
     if (!ctx || !buf) return NB_EINVAL;
     if (ctx->n_eval <= 0) return set_err(ctx, NB_ESTATE, "nb_get_forces: nothing evaluated");
+    NB_TRY(reserve_stage(ctx, 9 * (size_t)ctx->n_eval));
     NB_TRY(launch_f1_contig(ctx, ctx->n_eval, ctx->stage, false));
     return copy_out(ctx, buf, ctx->stage, 9 * (size_t)ctx->n_eval * sizeof(double));
 }
@@ -459,8 +504,12 @@ extern "C" int nb_set_forces(nb_ctx *ctx, const double *buf)
 {
     if (!ctx || !buf) return NB_EINVAL;
     if (ctx->n_eval <= 0) return set_err(ctx, NB_ESTATE, "nb_set_forces: nothing evaluated");
+    NB_TRY(reserve_stage(ctx, 9 * (size_t)ctx->n_eval));
     NB_TRY(copy_in(ctx, ctx->stage, buf, 9 * (size_t)ctx->n_eval * sizeof(double)));
-    return launch_f1_contig(ctx, ctx->n_eval, ctx->stage, true);
+    NB_TRY(launch_f1_contig(ctx, ctx->n_eval, ctx->stage, true));
+    // the caller stores the sums over all j-slices: the set just evaluated is now complete
+    if (ctx->eval_partial) { ctx->evaluated = true; ctx->eval_partial = false; }
+    return NB_OK;
 }
 
 extern "C" int nb_set_precision(nb_ctx *ctx, int mode)
@@ -468,14 +517,16 @@ extern "C" int nb_set_precision(nb_ctx *ctx, int mode)
     if (!ctx) return NB_EINVAL;
     if (mode != 0 && mode != 1) return set_err(ctx, NB_EINVAL, "nb_set_precision: 0 (FP64) or 1 (mixed SP/DP)");
     ctx->precision = mode;
-    ctx->evaluated = false;
+    ctx->evaluated = false; ctx->eval_partial = false;
     return NB_OK;
 }
 
 extern "C" int nb_set_loop_mode(nb_ctx *ctx, int device_driven)
 {
     if (!ctx) return NB_EINVAL;
-    if (device_driven < 0 || device_driven > 2) return set_err(ctx, NB_EINVAL, "nb_set_loop_mode: 0, 1 or 2");
+    if (device_driven < 0 || device_driven > 3) return set_err(ctx, NB_EINVAL, "nb_set_loop_mode: 0, 1, 2 or 3");
+    if (device_driven == 3 && ctx->N > RES_MAX_N)
+        return set_err(ctx, NB_EINVAL, "nb_set_loop_mode: mode 3 (cluster-resident loop) serves N <= %lld", (long long)RES_MAX_N);
     ctx->use_graph = device_driven;
     return NB_OK;
 }
@@ -493,8 +544,9 @@ extern "C" int nb_probe_fp64_peak(nb_ctx *ctx, int64_t iters, double *flops, flo
     return launch_probe(ctx, iters, flops, ms);
 }
 
-extern "C" int nb_probe_fp64_operands(nb_ctx *ctx, int mode, int64_t iters, double sm_mhz, double *cycles_per_inst)
+extern "C" int nb_set_debug(nb_ctx *ctx, int on)
 {
-    if (!ctx || iters < 1 || mode < 0 || mode > 5 || !(sm_mhz > 0.0)) return NB_EINVAL;
-    return launch_probe_operands(ctx, mode, iters, sm_mhz, cycles_per_inst);
+    if (!ctx) return NB_EINVAL;
+    ctx->debug = on ? 1 : 0;
+    return NB_OK;
 }

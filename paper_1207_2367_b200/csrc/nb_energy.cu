@@ -67,8 +67,9 @@ __global__ void __launch_bounds__(EN_THREADS)
             const double s = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
             double y = rsqrt_full(s);
             // pairs with j <= i belong to the other particle's sum; padded / massless records add
-            // nothing (integer test on the bits: +0.0 only, no FP64 pipe slot)
-            if (j0 + jj <= i || __double_as_longlong(b.y) == 0) y = 0.0;
+            // nothing, nor does a coincident pair at eps = 0 (s = +0: outside the domain, G12) -- integer
+            // tests on the bits, no FP64 pipe slot
+            if (j0 + jj <= i || __double_as_longlong(b.y) == 0 || __double_as_longlong(s) == 0) y = 0.0;
             p = fma(b.y, y, p);
         }
         pot += p;
@@ -110,124 +111,17 @@ __global__ void k_energy_final(const int nb, const double *__restrict__ part, do
     if (threadIdx.x == 0) out[0] = out[1] + out[2];
 }
 
-int launch_energy(nb_ctx *ctx, double out_host[9])
+int launch_energy(nb_ctx *ctx, const double *records, double out_host[9])
 {
     const int64_t N = ctx->N;
     const int nb = (int)((N + EN_THREADS - 1) / EN_THREADS);
     double *part = ctx->red;  // [nb][9] + 9
-    k_energy<<<nb, EN_THREADS, 0, ctx->stream>>>(N, ctx->Npad, ctx->eps2, ctx->jp, part + 9);
+    k_energy<<<nb, EN_THREADS, 0, ctx->stream>>>(N, ctx->Npad, ctx->eps2, records, part + 9);
     NB_LAUNCH_CHECK(ctx, "k_energy");
     k_energy_final<<<1, 256, 0, ctx->stream>>>(nb, part + 9, part);
     NB_LAUNCH_CHECK(ctx, "k_energy_final");
     NB_CUDA(ctx, cudaMemcpyAsync(out_host, part, 9 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     NB_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    return NB_OK;
-}
-
-// ---------------------------------------------------------------------------------------
-// DFMA-only probe: 16 independent FMA chains per thread, 8 warps per SM sub-partition.
-__global__ void __launch_bounds__(256, 4) k_probe_dfma(const long long iters, const double x0, double *__restrict__ sink)
-{
-    double a[16];
-#pragma unroll
-    for (int q = 0; q < 16; ++q) a[q] = x0 + q + threadIdx.x;
-    const double m = 0.999999, c = 1e-9;
-    for (long long it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int q = 0; q < 16; ++q) a[q] = fma(a[q], m, c);
-    }
-    double t = 0.0;
-#pragma unroll
-    for (int q = 0; q < 16; ++q) t += a[q];
-    if (t == 123.456) sink[0] = t;  // never true: keeps the chains alive
-}
-
-int launch_probe(nb_ctx *ctx, int64_t iters, double *flops, float *ms)
-{
-    cudaEvent_t e0, e1;
-    NB_CUDA(ctx, cudaEventCreate(&e0));
-    NB_CUDA(ctx, cudaEventCreate(&e1));
-    const int grid = ctx->n_sm * 4;
-    k_probe_dfma<<<grid, 256, 0, ctx->stream>>>(iters / 16 + 1, 1.0, ctx->red);  // warm-up
-    NB_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
-    k_probe_dfma<<<grid, 256, 0, ctx->stream>>>(iters, 1.0, ctx->red);
-    NB_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
-    NB_LAUNCH_CHECK(ctx, "k_probe_dfma");
-    ctx->n_launch += 1;
-    NB_CUDA(ctx, cudaEventSynchronize(e1));
-    float t = 0.f;
-    NB_CUDA(ctx, cudaEventElapsedTime(&t, e0, e1));
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    if (ms) *ms = t;
-    if (flops) *flops = 2.0 * 16.0 * (double)iters * 256.0 * (double)grid / ((double)t * 1e-3);
-    return NB_OK;
-}
-
-// Operand-fetch probe: 12 independent DFMA chains per thread, 24 DFMAs per loop trip, operands
-// pinned by inline PTX so that ptxas cannot fold them.
-template <int MODE>
-__global__ void __launch_bounds__(512) k_probe_operands(const long long iters, const double seed, double *__restrict__ sink)
-{
-    double x[12], a[12], b[12];
-    const double tf = (double)threadIdx.x;
-#pragma unroll
-    for (int k = 0; k < 12; ++k) {
-        x[k] = seed + k + tf;
-        // loaded, not computed: ptxas would otherwise re-materialise them inside the timed loop
-        a[k] = sink[1 + k] + tf * 1e-15;
-        b[k] = sink[13 + k] + tf * 1e-16;
-    }
-    for (long long it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int r = 0; r < 2; ++r) {
-#pragma unroll
-            for (int k = 0; k < 12; ++k) {
-                if (MODE == 0) asm volatile("fma.rn.f64 %0, %0, 0d3FEFFFFDE7210BE9, 0d3E112E0BE826D695;" : "+d"(x[k]));
-                if (MODE == 1) asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(x[k]) : "d"(a[k]), "d"(b[k]));
-                if (MODE == 2) asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(x[k]) : "d"(a[k / 3]), "d"(b[k]));
-                if (MODE == 3) asm volatile("fma.rn.f64 %0, %1, %1, %0;" : "+d"(x[k]) : "d"(a[k]));
-                if (MODE == 4) asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(x[k]) : "d"(a[0]), "d"(b[k]));
-                if (MODE == 5) {  // 3-register DFMA, then a DADD that shares one operand with it (1 fresh read)
-                    if (k % 2 == 0) asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(x[k]) : "d"(a[k]), "d"(b[k]));
-                    else asm volatile("add.f64 %0, %1, %0;" : "+d"(x[k]) : "d"(a[k - 1]));
-                }
-            }
-        }
-    }
-    double t = 0.0;
-#pragma unroll
-    for (int k = 0; k < 12; ++k) t += x[k];
-    if (t == 123.456) sink[0] = t;
-}
-
-int launch_probe_operands(nb_ctx *ctx, int mode, int64_t iters, double sm_mhz, double *cycles_per_inst)
-{
-    cudaEvent_t e0, e1;
-    NB_CUDA(ctx, cudaEventCreate(&e0));
-    NB_CUDA(ctx, cudaEventCreate(&e1));
-    const int grid = ctx->n_sm, threads = 512;  // 4 warps per SM sub-partition, as in the evaluation kernel
-    for (int pass = 0; pass < 2; ++pass) {
-        const long long n = pass ? iters : iters / 8 + 1;
-        if (pass) NB_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
-        switch (mode) {
-            case 0: k_probe_operands<0><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
-            case 1: k_probe_operands<1><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
-            case 2: k_probe_operands<2><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
-            case 3: k_probe_operands<3><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
-            case 4: k_probe_operands<4><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
-            default: k_probe_operands<5><<<grid, threads, 0, ctx->stream>>>(n, 1.0, ctx->red); break;
-        }
-        NB_LAUNCH_CHECK(ctx, "k_probe_operands");
-    }
-    NB_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
-    NB_CUDA(ctx, cudaEventSynchronize(e1));
-    float t = 0.f;
-    NB_CUDA(ctx, cudaEventElapsedTime(&t, e0, e1));
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    const double warp_inst_per_smsp = (double)iters * 24.0 * (threads / 32) / 4.0;
-    if (cycles_per_inst) *cycles_per_inst = (double)t * 1e-3 * sm_mhz * 1e6 / warp_inst_per_smsp;
     return NB_OK;
 }
 

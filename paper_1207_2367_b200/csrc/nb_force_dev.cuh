@@ -1,0 +1,300 @@
+// nb_force_dev.cuh -- device functions of the evaluation step, shared by the kernels of nb_force.cu
+// (one launch per evaluation, persistent form for the graph-driven loop) and nb_resident.cu (the
+// cluster-resident loop): the pair body (Eq. 8-10, with the Eq. 2 softening), the
+// mbarrier / bulk-copy primitives and force_item, the work of one (i-block, j-split) item.  All
+// drivers call the same functions with the same geometry, so their results are bit-identical.
+#pragma once
+#include "nb_internal.cuh"
+
+namespace nb {
+
+struct Acc9 {
+    double ax, ay, az, jx, jy, jz, sx, sy, sz;
+};
+
+__device__ __forceinline__ double rsqrt_seed(double s)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(s));
+    return y;
+}
+
+// One pair interaction, Eq. 8-10 in the factored form:
+//   s = |dr|^2 + eps^2, w = m_j s^(-3/2), g = -3 (dr.dv)/s, b3 = -3 beta,
+//   u = dv + g dr,  A0 = w dr,  A1 = w u,  A2 = w (da + 2 g u + b3 dr).
+// q points at the packed record {x y z vx vy vz ax ay az m} of particle j in shared memory.
+// SNAP = false (start-up pass 1, G8: only a and jerk are wanted; the snap of that pass would be
+// discarded): the a_ij differences, r.a, beta and the snap accumulation are left out -- 31 instead
+// of 53 FP64 instructions; a and jerk are computed by the same expressions.
+template <bool GUARD0, bool SNAP = true>
+__device__ __forceinline__ void pair_body(const double xi, const double yi, const double zi,
+                                          const double vxi, const double vyi, const double vzi,
+                                          const double axi, const double ayi, const double azi,
+                                          const double *__restrict__ q, const double eps2, Acc9 &A)
+{
+    const double2 p0 = *reinterpret_cast<const double2 *>(q);
+    const double2 p1 = *reinterpret_cast<const double2 *>(q + 2);
+    const double2 p2 = *reinterpret_cast<const double2 *>(q + 4);
+    const double2 p3 = *reinterpret_cast<const double2 *>(q + 6);
+    const double2 p4 = *reinterpret_cast<const double2 *>(q + 8);
+    // differences and the three dot products, component by component (z, y, x)
+    const double dvz = p2.y - vzi, dvy = p2.x - vyi, dvx = p1.y - vxi;
+    double vr = dvz * dvz;
+    vr = fma(dvy, dvy, vr);
+    vr = fma(dvx, dvx, vr);
+    const double dz = p1.x - zi, daz = p4.x - azi;
+    double s = fma(dz, dz, eps2);
+    double rv = dz * dvz;
+    vr = fma(dz, daz, vr);
+    const double dy = p0.y - yi, day = p3.y - ayi;
+    s = fma(dy, dy, s);
+    rv = fma(dy, dvy, rv);
+    vr = fma(dy, day, vr);
+    const double dx = p0.x - xi, dax = p3.x - axi;
+    s = fma(dx, dx, s);
+    rv = fma(dx, dvx, rv);
+    vr = fma(dx, dax, vr);
+    const double mj = p4.y;
+    double y0 = rsqrt_seed(s);
+    if (GUARD0) {  // eps = 0: a coincident pair (the self term) contributes nothing (G12)
+        if ((__double2hiint(s) | __double2loint(s)) == 0) y0 = 0.0;
+    }
+    // y = y0 (1 + e (1/2 + 3/8 e)), e = 1 - s y0^2: every instruction reads at most two registers
+    const double y2 = y0 * y0;
+    const double e = fma(-s, y2, 1.0);
+    const double p = fma(e, 0.375, 0.5);
+    const double ep1 = fma(e, p, 1.0);
+    const double y = y0 * ep1;         // s^(-1/2)
+    const double ri2 = y * y;          // 1/s
+    const double my = mj * y;
+    const double qq = ri2 * -3.0;
+    const double w = my * ri2;         // m_j s^(-3/2)
+    const double g = rv * qq;          // -3 alpha
+    const double qv = qq * vr;
+    const double gg = g * g;
+    const double g2 = g + g;
+    const double b3 = fma(gg, -1.0 / 3.0, qv);  // -3 beta = -3 (v^2 + r.a)/s - 3 alpha^2
+    const double ux = fma(g, dx, dvx), uy = fma(g, dy, dvy), uz = fma(g, dz, dvz);
+    A.ax = fma(w, dx, A.ax);
+    A.ay = fma(w, dy, A.ay);
+    A.az = fma(w, dz, A.az);
+    A.jx = fma(w, ux, A.jx);
+    A.jy = fma(w, uy, A.jy);
+    A.jz = fma(w, uz, A.jz);
+    if (!SNAP) return;  // everything that only feeds the snap above is dead code in this instantiation
+    double tx = fma(g2, ux, dax), ty = fma(g2, uy, day), tz = fma(g2, uz, daz);
+    tx = fma(b3, dx, tx);
+    ty = fma(b3, dy, ty);
+    tz = fma(b3, dz, tz);
+    A.sx = fma(w, tx, A.sx);
+    A.sy = fma(w, ty, A.sy);
+    A.sz = fma(w, tz, A.sz);
+}
+
+// The same pair in the paper's mixed precision (reading G27): the nine
+// differences are formed in double from the double records and rounded to float, everything
+// else of Eq. 8-10 is float arithmetic (FFMA/FMUL on the FP32 pipe, MUFU.RSQ), and the pair
+// terms are summed in float within one j-tile (the caller adds the tile sums in double).
+// FP64-pipe work per pair: 9 DADD + 10 F2F instead of 53 instructions.
+struct AccF {
+    float ax, ay, az, jx, jy, jz, sx, sy, sz;
+};
+template <bool GUARD0>
+__device__ __forceinline__ void pair_body_mx(const double xi, const double yi, const double zi,
+                                             const double vxi, const double vyi, const double vzi,
+                                             const double axi, const double ayi, const double azi,
+                                             const double *__restrict__ q, const float eps2, AccF &A)
+{
+    const double2 p0 = *reinterpret_cast<const double2 *>(q);
+    const double2 p1 = *reinterpret_cast<const double2 *>(q + 2);
+    const double2 p2 = *reinterpret_cast<const double2 *>(q + 4);
+    const double2 p3 = *reinterpret_cast<const double2 *>(q + 6);
+    const double2 p4 = *reinterpret_cast<const double2 *>(q + 8);
+    const float dx = (float)(p0.x - xi), dy = (float)(p0.y - yi), dz = (float)(p1.x - zi);
+    const float dvx = (float)(p1.y - vxi), dvy = (float)(p2.x - vyi), dvz = (float)(p2.y - vzi);
+    const float dax = (float)(p3.x - axi), day = (float)(p3.y - ayi), daz = (float)(p4.x - azi);
+    const float mj = (float)p4.y;
+    const float s = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, eps2)));
+    const float rv = fmaf(dx, dvx, fmaf(dy, dvy, dz * dvz));
+    const float vr = fmaf(dx, dax, fmaf(dy, day, fmaf(dz, daz, fmaf(dvx, dvx, fmaf(dvy, dvy, dvz * dvz)))));
+    float y = rsqrtf(s);
+    if (GUARD0) {  // eps = 0, or eps so small that m s^(-3/2) overflows a float (then w * 0 = NaN): the
+                   // self term (dr = 0 exactly, s = eps^2) is excluded explicitly (G12)
+        if (s == eps2) y = 0.0f;
+    }
+    const float P = y * y;             // 1/s
+    const float w = (mj * y) * P;      // m_j s^(-3/2)
+    const float qq = -3.0f * P;
+    const float g = rv * qq;           // -3 alpha
+    const float b3 = fmaf(g * g, -1.0f / 3.0f, qq * vr);  // -3 beta
+    const float g2 = g + g;
+    const float ux = fmaf(g, dx, dvx), uy = fmaf(g, dy, dvy), uz = fmaf(g, dz, dvz);
+    A.ax = fmaf(w, dx, A.ax); A.ay = fmaf(w, dy, A.ay); A.az = fmaf(w, dz, A.az);
+    A.jx = fmaf(w, ux, A.jx); A.jy = fmaf(w, uy, A.jy); A.jz = fmaf(w, uz, A.jz);
+    float tx = fmaf(g2, ux, dax), ty = fmaf(g2, uy, day), tz = fmaf(g2, uz, daz);
+    tx = fmaf(b3, dx, tx); ty = fmaf(b3, dy, ty); tz = fmaf(b3, dz, tz);
+    A.sx = fmaf(w, tx, A.sx); A.sy = fmaf(w, ty, A.sy); A.sz = fmaf(w, tz, A.sz);
+}
+
+// ---- mbarrier / bulk-copy primitives (PTX, sm_90+; SASS: SYNCS.*, UBLKCP) ---------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+            smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+
+// ---- the evaluation kernel -------------------------------------------------------------
+// One work item = (i-block ib, j-split sp): NT/JL i-particles against tiles [sp*tps, sp*tps+nt).
+// JLT = 1: one i per thread.  JLT = 0: JL (runtime, power of two <= 32) consecutive lanes share
+// one i and stride through the tile.  `tc` counts the tiles this CTA has consumed so far: ring
+// stage = tc & 1, mbarrier phase = (tc >> 1) & 1, so the ring carries over from item to item.
+// MX: 0 = FP64, 1 = mixed precision (reading G27), 2 = FP64 acceleration and jerk only
+// The NT threads that work on an item are a whole CTA (VS = 0: tid = threadIdx.x, block barrier) or a
+// "virtual CTA" inside a larger one (the resident loop of nb_resident.cu): one warp (VS = 1, warp barrier)
+// or NT = 128 threads on the named barrier `bar_id` (VS = 2).  The arithmetic and its order are the same.
+template <int VS>
+__device__ __forceinline__ void vcta_sync(const int bar_id, const int nthreads)
+{
+    if (VS == 0) __syncthreads();
+    else if (VS == 1) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "r"(nthreads) : "memory");
+}
+
+template <int NT, int TJ, int JLT, bool GUARD0, int MX, int UNR, int VS = 0>
+__device__ __forceinline__ void force_item(const double *__restrict__ jp, const double *__restrict__ jstream,
+                                           const int32_t *__restrict__ active, const int m, const int ib, const int sp, const int tiles_total,
+                                           const int tiles_per_split, const int JL, const double eps2,
+                                           double *__restrict__ out, const size_t cstride, const size_t sstride,
+                                           double (*tile)[TJ * REC], uint64_t *full, unsigned &tc,
+                                           const int tid_in = 0, const int bar_id = 0)
+{
+    constexpr int NS = 2;
+    constexpr uint32_t TILE_BYTES = TJ * REC * sizeof(double);
+    const int tid = VS == 0 ? (int)threadIdx.x : tid_in;
+    const int slots = NT / JL;              // i-particles per CTA
+    const int k = ib * slots + tid / JL;    // slot in the active list
+    const int jl = tid % JL;                // j-lane
+    const int t0 = sp * tiles_per_split;
+    const int nt = min(tiles_per_split, tiles_total - t0);
+    const char *src = reinterpret_cast<const char *>(jstream) + (size_t)t0 * TILE_BYTES;
+
+    if (tid == 0) {
+        for (int st = 0; st < NS && st < nt; ++st) {
+            const unsigned sg = (tc + st) & 1u;
+            mbar_expect_tx(&full[sg], TILE_BYTES);
+            bulk_g2s(tile[sg], src + (size_t)st * TILE_BYTES, TILE_BYTES, &full[sg]);
+        }
+    }
+
+    // i-particle: predicted r, v, a of active[k] (differences of PREDICTED data)
+    const int kc = min(k, m - 1);
+    const int i = active ? active[kc] : kc;
+    const double *pi = jp + (size_t)i * REC;
+    const double2 i0 = *reinterpret_cast<const double2 *>(pi);
+    const double2 i1 = *reinterpret_cast<const double2 *>(pi + 2);
+    const double2 i2 = *reinterpret_cast<const double2 *>(pi + 4);
+    const double2 i3 = *reinterpret_cast<const double2 *>(pi + 6);
+    const double i4 = pi[8];
+    const double xi = i0.x, yi = i0.y, zi = i1.x, vxi = i1.y, vyi = i2.x, vzi = i2.y;
+    const double axi = i3.x, ayi = i3.y, azi = i4;
+
+    // a warp whose slots are all beyond m only keeps the barriers company
+    const bool warp_idle = (ib * slots + (tid & ~31) / JL) >= m;
+
+    Acc9 T = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+    for (int it = 0; it < nt; ++it) {
+        const unsigned sg = tc & 1u;
+        mbar_wait(&full[sg], (tc >> 1) & 1u);
+        if (!warp_idle) {
+            const double *q = tile[sg];
+            if (MX == 1) {
+                AccF A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+                const float eps2f = (float)eps2;
+                if (JLT) {
+#pragma unroll 6
+                    for (int jj = 0; jj < TJ; ++jj)
+                        pair_body_mx<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2f, A);
+                } else {
+#pragma unroll 2
+                    for (int jj = jl; jj < TJ; jj += JL)
+                        pair_body_mx<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2f, A);
+                }
+                T.ax += (double)A.ax; T.ay += (double)A.ay; T.az += (double)A.az;
+                T.jx += (double)A.jx; T.jy += (double)A.jy; T.jz += (double)A.jz;
+                T.sx += (double)A.sx; T.sy += (double)A.sy; T.sz += (double)A.sz;
+            } else {
+                Acc9 A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+                if (JLT) {
+#pragma unroll UNR
+                    for (int jj = 0; jj < TJ; ++jj)
+                        pair_body<GUARD0, MX != 2>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
+                } else {
+#pragma unroll 2
+                    for (int jj = jl; jj < TJ; jj += JL)
+                        pair_body<GUARD0, MX != 2>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
+                }
+                T.ax += A.ax; T.ay += A.ay; T.az += A.az;
+                T.jx += A.jx; T.jy += A.jy; T.jz += A.jz;
+                T.sx += A.sx; T.sy += A.sy; T.sz += A.sz;
+            }
+        }
+        vcta_sync<VS>(bar_id, NT);  // every warp is done reading tile[sg]
+        if (tid == 0 && it + NS < nt) {
+            mbar_expect_tx(&full[sg], TILE_BYTES);
+            bulk_g2s(tile[sg], src + (size_t)(it + NS) * TILE_BYTES, TILE_BYTES, &full[sg]);
+        }
+        ++tc;
+    }
+
+    if (!JLT) {  // fixed-order butterfly over the JL lanes that share this i
+        for (int off = JL >> 1; off > 0; off >>= 1) {
+            T.ax += __shfl_xor_sync(0xffffffffu, T.ax, off);
+            T.ay += __shfl_xor_sync(0xffffffffu, T.ay, off);
+            T.az += __shfl_xor_sync(0xffffffffu, T.az, off);
+            T.jx += __shfl_xor_sync(0xffffffffu, T.jx, off);
+            T.jy += __shfl_xor_sync(0xffffffffu, T.jy, off);
+            T.jz += __shfl_xor_sync(0xffffffffu, T.jz, off);
+            T.sx += __shfl_xor_sync(0xffffffffu, T.sx, off);
+            T.sy += __shfl_xor_sync(0xffffffffu, T.sy, off);
+            T.sz += __shfl_xor_sync(0xffffffffu, T.sz, off);
+        }
+    }
+    if (k < m && jl == 0) {
+        double *o = out + (size_t)sp * sstride + k;
+        o[0 * cstride] = T.ax; o[1 * cstride] = T.ay; o[2 * cstride] = T.az;
+        o[3 * cstride] = T.jx; o[4 * cstride] = T.jy; o[5 * cstride] = T.jz;
+        o[6 * cstride] = T.sx; o[7 * cstride] = T.sy; o[8 * cstride] = T.sz;
+    }
+}
+
+}  // namespace nb

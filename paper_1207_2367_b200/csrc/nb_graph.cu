@@ -102,7 +102,7 @@ int graph_run(nb_ctx *ctx, double t_end, int64_t max_steps, int64_t *n_steps)
     ctx->n_steps += h->n_steps;
     ctx->n_pairs += h->n_pairs;
     for (int b = 0; b < 64; ++b) ctx->hist[b] += h->hist[b];
-    ctx->have_block = false; ctx->evaluated = false;
+    ctx->have_block = false; ctx->evaluated = false; ctx->eval_partial = false;
     if (n_steps) *n_steps = h->n_steps;
     return NB_OK;
 }

@@ -83,6 +83,8 @@ constexpr int NT_B = 32, TJ_B = 64, MINB_B = 16;    // variant B: one warp per C
 constexpr int64_t L2_CHUNK_BYTES = 24 << 20;         // j-stream piece kept L2-resident across i-block waves
 constexpr int GEOM_CACHE_M = 4096;                   // the device loop remembers the geometry of set sizes up to this
 constexpr int MAX_WAVES = 64;                       // the split search considers 1..MAX_WAVES waves
+constexpr int64_t RES_MAX_N = 16384;                 // the cluster-resident loop (nb_resident.cu) serves N up to this
+constexpr int64_t RES_AUTO_N = 2048;                 // ... and is the default driver up to this
 
 // Number of j-splits.  All CTAs do the same work per tile, so the cost of a launch is
 // waves x (tiles per split + a fixed per-CTA cost of 0.75 tile) + 0.002 S, in integer
@@ -181,7 +183,9 @@ struct nb_ctx {
     bool pred_valid;   // predicted stream holds data
     double t_pred;     // time of the predicted stream
     bool have_block;   // nb_next_block selected a set that is not yet committed
-    bool evaluated;    // nb_force evaluated the scheduler's set at t_next
+    bool evaluated;    // nb_force evaluated the scheduler's set at t_next (complete sums: corrector may run)
+    bool eval_partial; // the same, but over a proper j-slice: becomes `evaluated` when nb_set_forces stores the reduced sums
+    int debug;         // nb_set_debug: range-check caller-supplied index lists
     double t_now, t_next;
     int64_t n_active;       // scheduler's set
     int64_t n_eval;         // size of the last evaluated set
@@ -193,7 +197,9 @@ struct nb_ctx {
     int32_t *active;                // [Npad] scheduler's list
     int32_t *user_idx;              // [Npad] copy of a caller-supplied list
     double *f1;                     // [9][Npad]
-    double *stage;                  // [9*Npad] staging for [n][3] in/out copies
+    double *stage;                  // staging for [n][3] / [n][21] in/out copies and the scratch prediction of
+                                    // nb_energy; stage_cap doubles, grown on demand (reserve_stage)
+    size_t stage_cap;
     double *partials;               // [S][9][mpad]
     size_t partials_cap;            // in doubles (grown on demand up to partials_limit)
     size_t partials_limit;          // most the split search can ask for: bounds S in choose_geom
@@ -201,6 +207,7 @@ struct nb_ctx {
     int32_t *blk_count;             // per-block match counts / offsets
     int64_t n_sched_blocks;
     double *red;                    // reduction scratch (energy)
+    int32_t *h_dbg, *d_dbg;         // pinned, mapped {number of bad indices, first bad slot} of the debug check
     nb::Sched *h_sched;             // pinned host mirror
     nb::Sched *d_sched;             // device alias of h_sched
     nb::StepCtl *ctl;               // device control block of the graph-driven block-step loop
@@ -210,7 +217,8 @@ struct nb_ctx {
     int graph_batch;
     int graph_split, graph_jlanes, graph_precision;  // knobs the captured graph was built with
     int64_t launches_per_batch;     // kernels in one replay of step_graph
-    int use_graph;                  // 1, 2: nb_run_until / nb_run_steps drive the loop from the device (2: with PDL)
+    int use_graph;                  // loop mode: 0 host-issued calls; 1, 2 graph batches (2: with PDL); 3 cluster-resident loop
+    int res_cluster;                // CTAs of the resident loop's cluster (16, or 8 where 16 cannot be scheduled)
     int graph_pdl;                  // the captured graph uses programmatic dependent launch
 
     // tuning
@@ -233,9 +241,11 @@ namespace nb {
 
 // ----- nb_force.cu
 // Evaluate (acc, jerk, snap) of `m` particles (active == nullptr: particles 0..m-1) against the
-// Npad predicted records; result in ctx->f1[c][k].  with_snap = false skips nothing in the
-// arithmetic (the body is the same); it only exists for symmetry of the start-up passes.
+// Npad predicted records; result in ctx->f1[c][k].  no_snap = true (start-up pass 1, G8) launches the
+// SNAP = false instantiation of the pair body: acceleration and jerk only, 31 instead of 53 FP64
+// instructions per pair; the snap planes of f1 are then written as zeros.
 int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m, bool no_snap = false);
+int launch_check_indices(nb_ctx *ctx, const int32_t *idx, int64_t m);   // debug: fills ctx->h_dbg (after a sync)
 int query_force_occupancy(nb_ctx *ctx);
 int enqueue_force_persistent(nb_ctx *ctx);   // both variants + reduction; set size and geometry come from ctx->ctl
 // f1[c][k] -> out[q][k][3] (q = 0 acc, 1 jerk, 2 snap) contiguous in ctx->stage
@@ -245,7 +255,7 @@ int reserve_partials(nb_ctx *ctx, size_t doubles);
 
 // ----- nb_step.cu
 int launch_load_state(nb_ctx *ctx, const double *pos_dev, const double *vel_dev, const double *mass_dev);
-int launch_predict(nb_ctx *ctx, double t);
+int launch_predict(nb_ctx *ctx, double t, double *records = nullptr);   // records: destination (default ctx->jp)
 int launch_set_pred(nb_ctx *ctx, const double *pos, const double *vel, const double *acc, bool pos_vel, bool acc_valid);
 int launch_get_pred(nb_ctx *ctx, double *pos, double *vel, double *acc);
 int launch_pack3(nb_ctx *ctx, const double *soa, double *aos);      // [3][Npad] -> [N][3]
@@ -263,12 +273,17 @@ int launch_graph_begin(nb_ctx *ctx, double t_end, int64_t steps);    // seeds ct
 int graph_run(nb_ctx *ctx, double t_end, int64_t max_steps, int64_t *n_steps);
 void graph_release(nb_ctx *ctx);
 
+// ----- nb_resident.cu
+int resident_run(nb_ctx *ctx, double t_end, int64_t max_steps, int64_t *n_steps);
+
 // ----- nb_energy.cu
-int launch_energy(nb_ctx *ctx, double out_host[9]);
+int launch_energy(nb_ctx *ctx, const double *records, double out_host[9]);
 
 // ----- nb_probe.cu
 int launch_probe(nb_ctx *ctx, int64_t iters, double *flops, float *ms);
-int launch_probe_operands(nb_ctx *ctx, int mode, int64_t iters, double sm_mhz, double *cycles_per_inst);
+
+// ----- nb_api.cu
+int reserve_stage(nb_ctx *ctx, size_t doubles);
 
 int set_err(nb_ctx *ctx, int code, const char *fmt, ...);
 

@@ -21,7 +21,7 @@ __all__ = [
     "nb_force", "nb_correct_and_step", "nb_run_until", "nb_run_steps", "nb_energy", "nb_get_state",
     "nb_get_derivs", "nb_get_pred", "nb_set_pred_acc", "nb_set_pred", "nb_get_full_state",
     "nb_set_full_state", "nb_get_stats", "nb_set_tuning", "nb_set_loop_mode", "nb_set_precision", "nb_set_j_range", "nb_get_forces", "nb_set_forces", "nb_get_launch", "nb_probe_fp64_peak",
-    "nb_probe_fp64_operands", "nb_version", "nb_last_error",
+    "nb_set_debug", "nb_version", "nb_last_error",
 ]
 
 NB_OK, NB_EINVAL, NB_ESTATE, NB_ECUDA, NB_ENOMEM = 0, -1, -2, -3, -4
@@ -66,7 +66,7 @@ _SIGS = {
     "nb_set_forces": (C.c_int, [_vp, _vp]),
     "nb_get_launch": (C.c_int, [_vp, C.POINTER(_i64)]),
     "nb_probe_fp64_peak": (C.c_int, [_vp, _i64, C.POINTER(_dbl), C.POINTER(C.c_float)]),
-    "nb_probe_fp64_operands": (C.c_int, [_vp, C.c_int, _i64, _dbl, C.POINTER(_dbl)]),
+    "nb_set_debug": (C.c_int, [_vp, C.c_int]),
     "nb_last_error": (C.c_char_p, [_vp]),
     "nb_free": (None, [_vp]),
     "nb_version": (C.c_char_p, []),
@@ -298,10 +298,8 @@ def nb_probe_fp64_peak(ctx, iters=1 << 16):
     return f.value, ms.value
 
 
-def nb_probe_fp64_operands(ctx, mode, iters=20000, sm_mhz=1965.0):
-    c = _dbl()
-    _check(ctx, lib().nb_probe_fp64_operands(ctx, int(mode), int(iters), float(sm_mhz), C.byref(c)))
-    return c.value
+def nb_set_debug(ctx, on=1):
+    _check(ctx, lib().nb_set_debug(ctx, int(on)))
 
 
 # ---------------------------------------------------------------------------- convenience wrapper

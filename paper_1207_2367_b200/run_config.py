@@ -188,29 +188,18 @@ def run_fig1(nb, Ns, etas, t_end=4.5, every=0.5, eps=1e-4):
 
 
 def run_probe(nb):
-    """DFMA peak and operand-fetch probes on a tiny context."""
-    import subprocess
+    """DFMA-only peak probe on a tiny context (the measured denominator beside the derived FP64 peak)."""
     z = np.zeros((128, 3)); z[:, 0] = np.arange(128)
     g = nb.NBody(_dev(z), _dev(z), _dev(np.ones(128)), 1e-3, 0.45)
-    try:
-        mhz = float(subprocess.run(["nvidia-smi", "--query-gpu=clocks.max.sm", "--format=csv,noheader,nounits", "-i", "0"],
-                                   capture_output=True, text=True).stdout.split()[0])
-    except Exception:
-        mhz = 1965.0
     f, ms = nb.nb_probe_fp64_peak(g.ctx, 1 << 17)
-    names = {0: "1 register + immediates", 1: "3 distinct registers", 2: "3 registers, one shared by 3 consecutive DFMAs",
-             3: "2 distinct registers (a*a+c)", 4: "3 registers, one shared by all DFMAs",
-             5: "3-register DFMA alternating with a DADD sharing one source (per FP64 instruction)"}
-    out = {"sm_mhz_assumed": mhz, "dfma_peak_tflops": f / 1e12, "nominal_tflops": PEAK / 1e12,
-           "cycles_per_warp_inst_per_smsp": {names[k]: nb.nb_probe_fp64_operands(g.ctx, k, 20000, mhz) for k in range(6)}}
     g.close()
-    return out
+    return {"dfma_peak_tflops": f / 1e12, "nominal_tflops": PEAK / 1e12, "ms": ms}
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", type=int, default=None, choices=[1, 2, 3, 4, 5])
-    ap.add_argument("--probe", action="store_true", help="FP64 pipe probes only (DESIGN.md section 6.3)")
+    ap.add_argument("--probe", action="store_true", help="DFMA-only FP64 peak probe (DESIGN.md section 7)")
     ap.add_argument("--n", type=int, default=None, help="override N (smaller dry runs)")
     ap.add_argument("--t-end", type=float, default=None)
     ap.add_argument("--steps", type=int, default=None)
