@@ -25,13 +25,13 @@
 namespace nb {
 
 // grid.x: i-blocks, grid.y: j-splits; geometry passed by the host.
-template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int MX = 0, int UNR = 12>
-__global__ void __launch_bounds__(NT, MINB)
+template <int JL, bool GUARD0, int MX = 0, int UNR = 12>
+__global__ void __launch_bounds__(NT_E, MINB_E)
     k_force(const double *__restrict__ jp, const double *__restrict__ jstream,
-            const int32_t *__restrict__ active, const int m, const int tiles_total, const int tiles_per_split, const int JLr, const double eps2,
-            double *__restrict__ out, const size_t cstride, const size_t sstride)
+            const int32_t *__restrict__ active, const int m, const int tiles_total, const int tiles_per_split, const double eps2,
+            double *__restrict__ out, const size_t cstride, const size_t kstride, const size_t sstride)
 {
-    __shared__ __align__(128) double tile[2][TJ * REC];
+    __shared__ __align__(128) double tile[2][TJ_E * REC];
     __shared__ __align__(8) uint64_t full[2];
     if (threadIdx.x == 0) {
         mbar_init(&full[0], 1);
@@ -40,8 +40,8 @@ __global__ void __launch_bounds__(NT, MINB)
     }
     __syncthreads();
     unsigned tc = 0;
-    force_item<NT, TJ, JLT, GUARD0, MX, UNR>(jp, jstream, active, m, blockIdx.x, blockIdx.y, tiles_total, tiles_per_split,
-                                         JLT ? 1 : JLr, eps2, out, cstride, sstride, tile, full, tc);
+    force_item<NT_E, TJ_E, JL, GUARD0, MX, UNR>(jp, jstream, active, m, blockIdx.x, blockIdx.y, tiles_total, tiles_per_split,
+                                                eps2, out, cstride, kstride, sstride, tile, full, tc);
 }
 
 // Persistent form for the device-driven block-step loop (nb_graph.cu): a fixed grid of
@@ -50,16 +50,16 @@ __global__ void __launch_bounds__(NT, MINB)
 // from a counter in the control block (items of one launch take equally long, but CTAs do not start
 // together: a fixed stride left a 2 % tail at m ~ 2e5).  Item w is (i-block w % n_ib, split
 // w / n_ib), so concurrently running CTAs stream the same j-split.
-template <int NT, int TJ, int MINB, int JLT, bool GUARD0, int MX = 0, int UNR = 12>
-__global__ void __launch_bounds__(NT, MINB)
+template <bool GUARD0, int MX = 0, int UNR = 12>
+__global__ void __launch_bounds__(NT_E, MINB_E)
     k_force_persistent(const double *__restrict__ jp, const int32_t *__restrict__ active_list, const int64_t N,
                        const int64_t Npad, const double eps2, double *__restrict__ f1,
                        double *__restrict__ partials, StepCtl *__restrict__ ctl)
 {
     pdl_trigger();
     pdl_wait();
-    if (ctl->done || ctl->g.variant != (JLT ? 0 : 1)) return;
-    __shared__ __align__(128) double tile[2][TJ * REC];
+    if (ctl->done) return;
+    __shared__ __align__(128) double tile[2][TJ_E * REC];
     __shared__ __align__(8) uint64_t full[2];
     __shared__ long long next_item;
     if (threadIdx.x == 0) {
@@ -72,15 +72,14 @@ __global__ void __launch_bounds__(NT, MINB)
     const ForceGeom g = ctl->g;
     const int32_t *active = (m == N) ? nullptr : active_list;
     double *out = g.S > 1 ? partials : f1;
-    const size_t cstride = g.S > 1 ? (size_t)g.mpad : (size_t)Npad;
-    const size_t sstride = 9 * (size_t)g.mpad;
-    const int tiles_total = (int)(Npad / TJ);
+    const PartLayout L = part_layout(g.S, g.mpad, Npad);
+    const int tiles_total = (int)(Npad / TJ_E);
     const long long items = (long long)g.n_ib * g.S;
     unsigned tc = 0;
     long long w = blockIdx.x;
     while (w < items) {
-        force_item<NT, TJ, JLT, GUARD0, MX, UNR>(jp, jp, active, m, (int)(w % g.n_ib), (int)(w / g.n_ib), tiles_total,
-                                                 g.tps, g.JL, eps2, out, cstride, sstride, tile, full, tc);
+        force_item_jl<NT_E, TJ_E, GUARD0, MX, UNR>(g.JL, jp, jp, active, m, (int)(w % g.n_ib), (int)(w / g.n_ib), tiles_total,
+                                                   g.tps, eps2, out, L.cstride, L.kstride, L.sstride, tile, full, tc);
         if (threadIdx.x == 0) next_item = (long long)gridDim.x + atomicAdd(&ctl->work, 1u);
         __syncthreads();
         w = next_item;
@@ -88,8 +87,8 @@ __global__ void __launch_bounds__(NT, MINB)
     }
 }
 
-// ---- partial-sum reduction (Table 1 row 4): f1[c][k] = sum_s part[s][c][k], s ascending ---
-// thread-per-element version: coalesced along k, used when the number of splits is small
+// ---- partial-sum reduction (Table 1 row 4): f1[c][k] = sum over the splits, fixed order (part_layout) ---
+// fewer than 32 splits: one thread per element, coalesced along k
 __global__ void k_reduce_thread(const double *__restrict__ part, const int S, const int m,
                                 const size_t cstride, const size_t sstride, double *__restrict__ f1,
                                 const size_t f1stride)
@@ -97,24 +96,18 @@ __global__ void k_reduce_thread(const double *__restrict__ part, const int S, co
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const int c = blockIdx.y;
     if (k >= m) return;
-    const double *p = part + c * cstride + k;
-    double acc = 0.0;
-    for (int s = 0; s < S; ++s) acc += p[(size_t)s * sstride];
-    f1[c * f1stride + k] = acc;
+    f1[c * f1stride + k] = sum_splits_thread(part + c * cstride + k, S, sstride);
 }
-// warp-per-element version: lane l sums splits l, l+32, ... then a fixed butterfly
+// 32 splits or more: one warp per element, the S values of an element are consecutive
 __global__ void k_reduce_warp(const double *__restrict__ part, const int S, const int m,
-                              const size_t cstride, const size_t sstride, double *__restrict__ f1,
+                              const size_t cstride, const size_t kstride, double *__restrict__ f1,
                               const size_t f1stride)
 {
     const int wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (wid >= 9 * m) return;
     const int c = wid / m, k = wid - c * m;
-    const double *p = part + c * cstride + k;
-    double acc = 0.0;
-    for (int s = lane; s < S; s += 32) acc += p[(size_t)s * sstride];
-    for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+    const double acc = sum_splits_warp(part + c * cstride + (size_t)k * kstride, S, lane);
     if (lane == 0) f1[c * f1stride + k] = acc;
 }
 
@@ -131,49 +124,13 @@ __global__ void k_unpack_f1(const double *__restrict__ f1, const size_t f1stride
     }
 }
 
-// Reduction for the device-driven loop: fixed grid, sizes read from the control block.  Element
-// e = c * m + k; the sum over splits runs in ascending split order exactly as in k_reduce_thread
-// (S < 32) or k_reduce_warp (S >= 32), so both drivers give bit-identical results.
-__global__ void __launch_bounds__(256)
-    k_reduce_persistent(const double *__restrict__ part, const StepCtl *__restrict__ ctl, double *__restrict__ f1,
-                        const size_t f1stride)
-{
-    pdl_trigger();
-    pdl_wait();
-    if (ctl->done || ctl->g.S <= 1) return;
-    const int S = ctl->g.S, m = (int)ctl->n_active;
-    const size_t cstride = (size_t)ctl->g.mpad, sstride = 9 * (size_t)ctl->g.mpad;
-    const long long total = 9LL * m;
-    if (S < 32) {
-        for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
-            const int c = (int)(e / m), k = (int)(e - (long long)c * m);
-            const double *p = part + c * cstride + k;
-            double acc = 0.0;
-            for (int s = 0; s < S; ++s) acc += p[(size_t)s * sstride];
-            f1[c * f1stride + k] = acc;
-        }
-    } else {
-        const int lane = threadIdx.x & 31;
-        const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
-        for (long long wid = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; wid < total; wid += nwarps) {
-            const int c = (int)(wid / m), k = (int)(wid - (long long)c * m);
-            const double *p = part + c * cstride + k;
-            double acc = 0.0;
-            for (int s = lane; s < S; s += 32) acc += p[(size_t)s * sstride];
-            for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
-            if (lane == 0) f1[c * f1stride + k] = acc;
-        }
-    }
-}
-
 // ---- host side ---------------------------------------------------------------------------
-// The split search never asks for more than MAX_WAVES waves of CTAs, i.e. S * m <= MAX_WAVES x
-// (resident CTAs) x (i-slots per CTA); S <= 65535 splits of mpad <= m + 31 add the slack term.
+// The split search never asks for more than MAX_WAVES waves of CTAs, i.e. S * n_ib <= MAX_WAVES x
+// (resident CTAs), each i-block of NT_E / JL >= 4 slots; S <= 65535 splits of mpad <= m + 31 add the slack term.
 static size_t partials_bound(const nb_ctx *ctx)
 {
-    const int64_t a = (int64_t)ctx->n_sm * ctx->occ[0] * NT_A, b = (int64_t)ctx->n_sm * ctx->occ[1] * NT_B;
-    int64_t items = (int64_t)MAX_WAVES * (a > b ? a : b) + 32 * 65536;
-    const int64_t by_n = (ctx->Npad / TJ_B) * (ctx->Npad + 32);   // S <= tiles, mpad <= Npad + 32
+    int64_t items = (int64_t)MAX_WAVES * ctx->n_sm * ctx->occ[0] * NT_E + 32 * 65536;
+    const int64_t by_n = (ctx->Npad / TJ_E) * (ctx->Npad + 32);   // S <= tiles, mpad <= Npad + 32
     if (by_n < items) items = by_n;
     return (size_t)(9 * items);
 }
@@ -181,18 +138,10 @@ static size_t partials_bound(const nb_ctx *ctx)
 int query_force_occupancy(nb_ctx *ctx)
 {
     int v = 0;
-    NB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
-                     &v, k_force<NT_A, TJ_A, MINB_A, 1, false>, NT_A, 0));
+    NB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_force<1, false>, NT_E, 0));
     ctx->occ[0] = v > 0 ? v : 1;
-    NB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
-                     &v, k_force<NT_B, TJ_B, MINB_B, 0, false>, NT_B, 0));
+    NB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_force_persistent<false>, NT_E, 0));
     ctx->occ[1] = v > 0 ? v : 1;
-    NB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
-                     &v, k_force_persistent<NT_A, TJ_A, MINB_A, 1, false>, NT_A, 0));
-    ctx->occ[2] = v > 0 ? v : 1;
-    NB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(
-                     &v, k_force_persistent<NT_B, TJ_B, MINB_B, 0, false>, NT_B, 0));
-    ctx->occ[3] = v > 0 ? v : 1;
     ctx->partials_limit = partials_bound(ctx);
     return NB_OK;
 }
@@ -214,21 +163,22 @@ int reserve_partials(nb_ctx *ctx, size_t need)
 // eps^2 ~ 1e-24 that product overflows, so the self pair is then excluded by the guard variant.
 static bool mx_needs_guard(const nb_ctx *ctx) { return (float)ctx->eps2 < 1e-24f; }
 
-template <int NT, int TJ, int MINB, int JLT>
-static void launch_variant(nb_ctx *ctx, dim3 grid, const int32_t *active, int m, int tiles_total,
-                           int tps, int JL, double *out, size_t cstride, size_t sstride, bool no_snap)
+template <int JL>
+static void launch_lanes(nb_ctx *ctx, dim3 grid, const int32_t *active, int m, int tiles_total, int tps,
+                         double *out, const PartLayout &L, bool no_snap)
 {
     const double *jstream = ctx->jp + (size_t)ctx->j_begin * REC;   // j-shard (nb_set_j_range), else the whole stream
-#define NB_KF(G0, MXP)                                                                 \
-    k_force<NT, TJ, MINB, JLT, G0, MXP><<<grid, NT, 0, ctx->stream>>>(ctx->jp, jstream, active, m, tiles_total, tps, JL, \
-                                                                      ctx->eps2, out, cstride, sstride)
+#define NB_KF(G0, MXP)                                                                                              \
+    k_force<JL, G0, MXP><<<grid, NT_E, 0, ctx->stream>>>(ctx->jp, jstream, active, m, tiles_total, tps, ctx->eps2, out, \
+                                                          L.cstride, L.kstride, L.sstride)
     const bool mx = ctx->precision == 1;
     const bool g0 = mx ? mx_needs_guard(ctx) : ctx->eps == 0.0;
     if (g0 && mx) NB_KF(true, 1);
     else if (mx) NB_KF(false, 1);
-    else if (g0 && no_snap) NB_KF(true, 2);
-    else if (no_snap) NB_KF(false, 2);
-    else if (g0) NB_KF(true, 0);
+    else if (JL == 1 && no_snap) {     // start-up pass 1 of a large system; small ones take the full body (same a, jerk)
+        if (g0) NB_KF(true, 2);
+        else NB_KF(false, 2);
+    } else if (g0) NB_KF(true, 0);
     else NB_KF(false, 0);
 #undef NB_KF
 }
@@ -238,53 +188,49 @@ int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m, bool no_snap)
     if (m <= 0) return NB_OK;
     // records of the j-shard, padded to whole tiles (records N..Npad-1 have zero mass)
     const int64_t jlen = (ctx->j_end == ctx->N ? ctx->Npad : ctx->j_end) - ctx->j_begin;
-    const ForceGeom g = choose_geom(m, jlen, ctx->n_sm, ctx->occ[0], ctx->occ[1], (int64_t)ctx->partials_limit,
+    const ForceGeom g = choose_geom(m, jlen, ctx->n_sm, ctx->occ[0], (int64_t)ctx->partials_limit,
                                     ctx->force_split, ctx->force_jlanes);
-    const bool varA = g.variant == 0;
-    const int TJ = varA ? TJ_A : TJ_B;
-    const int64_t tiles = jlen / TJ;
+    const int64_t tiles = jlen / TJ_E;
     double *out = ctx->f1;
-    size_t cstride = (size_t)ctx->Npad, sstride = 0;
     if (g.S > 1) {
         const int rc = reserve_partials(ctx, (size_t)g.S * 9 * (size_t)g.mpad);
         if (rc != NB_OK) return rc;
-        out = ctx->partials; cstride = (size_t)g.mpad; sstride = 9 * (size_t)g.mpad;
+        out = ctx->partials;
     }
+    const PartLayout L = part_layout(g.S, g.mpad, ctx->Npad);
     dim3 grid((unsigned)g.n_ib, (unsigned)g.S, 1);
-    if (varA)
-        launch_variant<NT_A, TJ_A, MINB_A, 1>(ctx, grid, active, (int)m, (int)tiles, g.tps, 1, out, cstride, sstride, no_snap);
-    else
-        launch_variant<NT_B, TJ_B, MINB_B, 0>(ctx, grid, active, (int)m, (int)tiles, g.tps, g.JL, out, cstride, sstride, no_snap);
+    switch (g.JL) {
+        case 1: launch_lanes<1>(ctx, grid, active, (int)m, (int)tiles, g.tps, out, L, no_snap); break;
+        case 2: launch_lanes<2>(ctx, grid, active, (int)m, (int)tiles, g.tps, out, L, no_snap); break;
+        case 4: launch_lanes<4>(ctx, grid, active, (int)m, (int)tiles, g.tps, out, L, no_snap); break;
+        case 8: launch_lanes<8>(ctx, grid, active, (int)m, (int)tiles, g.tps, out, L, no_snap); break;
+        case 16: launch_lanes<16>(ctx, grid, active, (int)m, (int)tiles, g.tps, out, L, no_snap); break;
+        default: launch_lanes<32>(ctx, grid, active, (int)m, (int)tiles, g.tps, out, L, no_snap); break;
+    }
     NB_LAUNCH_CHECK(ctx, "k_force");
     if (g.S > 1) {
         if (g.S < 32) {
             dim3 gr((unsigned)((m + 127) / 128), 9, 1);
-            k_reduce_thread<<<gr, 128, 0, ctx->stream>>>(out, g.S, (int)m, cstride, sstride, ctx->f1, (size_t)ctx->Npad);
+            k_reduce_thread<<<gr, 128, 0, ctx->stream>>>(out, g.S, (int)m, L.cstride, L.sstride, ctx->f1, (size_t)ctx->Npad);
         } else {
             const int64_t warps = 9 * m;
-            k_reduce_warp<<<(unsigned)((warps + 7) / 8), 256, 0, ctx->stream>>>(out, g.S, (int)m, cstride, sstride, ctx->f1, (size_t)ctx->Npad);
+            k_reduce_warp<<<(unsigned)((warps + 7) / 8), 256, 0, ctx->stream>>>(out, g.S, (int)m, L.cstride, L.kstride, ctx->f1, (size_t)ctx->Npad);
         }
         NB_LAUNCH_CHECK(ctx, "k_reduce");
     }
-    ctx->last_launch[0] = varA ? NT_A : NT_B; ctx->last_launch[1] = g.JL; ctx->last_launch[2] = g.S;
-    ctx->last_launch[3] = (int64_t)g.n_ib * g.S; ctx->last_launch[4] = TJ;
+    ctx->last_launch[0] = NT_E; ctx->last_launch[1] = g.JL; ctx->last_launch[2] = g.S;
+    ctx->last_launch[3] = (int64_t)g.n_ib * g.S; ctx->last_launch[4] = TJ_E;
     ctx->n_pairs += (double)m * (double)(ctx->j_end - ctx->j_begin);
     return NB_OK;
 }
 
-// Device-driven loop: both variants are enqueued with fixed grids (one wave of resident CTAs);
-// the one the gather kernel did not select returns at once, as does everything when the control
-// block says `done`.
+// Device-driven loop: one wave of resident CTAs; everything returns at once when the control block says `done`.
 int enqueue_force_persistent(nb_ctx *ctx)
 {
-    const unsigned gA = (unsigned)(ctx->n_sm * ctx->occ[2]), gB = (unsigned)(ctx->n_sm * ctx->occ[3]);
-#define NB_KP(G0, MXP)                                                                                       \
-    do {                                                                                                     \
-        launch_chain(k_force_persistent<NT_A, TJ_A, MINB_A, 1, G0, MXP>, dim3(gA), dim3(NT_A), ctx->stream, pdl, \
-                     ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);   \
-        launch_chain(k_force_persistent<NT_B, TJ_B, MINB_B, 0, G0, MXP>, dim3(gB), dim3(NT_B), ctx->stream, pdl, \
-                     ctx->jp, ctx->active, ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl);   \
-    } while (0)
+    const unsigned gP = (unsigned)(ctx->n_sm * ctx->occ[1]);
+#define NB_KP(G0, MXP)                                                                                      \
+    launch_chain(k_force_persistent<G0, MXP>, dim3(gP), dim3(NT_E), ctx->stream, pdl, ctx->jp, ctx->active, \
+                 ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl)
     const bool mx = ctx->precision == 1, pdl = ctx->use_graph == 2;
     const bool g0 = mx ? mx_needs_guard(ctx) : ctx->eps == 0.0;
     if (g0 && mx) NB_KP(true, 1);
@@ -293,10 +239,6 @@ int enqueue_force_persistent(nb_ctx *ctx)
     else NB_KP(false, 0);
 #undef NB_KP
     NB_LAUNCH_CHECK(ctx, "k_force_persistent");
-    ctx->n_launch += 1;  // two kernels
-    launch_chain(k_reduce_persistent, dim3((unsigned)(2 * ctx->n_sm)), dim3(256), ctx->stream, pdl, ctx->partials,
-                 ctx->ctl, ctx->f1, (size_t)ctx->Npad);
-    NB_LAUNCH_CHECK(ctx, "k_reduce_persistent");
     return NB_OK;
 }
 

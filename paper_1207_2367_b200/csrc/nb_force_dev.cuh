@@ -136,6 +136,10 @@ __device__ __forceinline__ void pair_body_mx(const double xi, const double yi, c
     A.sx = fmaf(w, tx, A.sx); A.sy = fmaf(w, ty, A.sy); A.sz = fmaf(w, tz, A.sz);
 }
 
+#ifndef NB_PAIR_BODY
+#define NB_PAIR_BODY pair_body
+#endif
+
 // ---- mbarrier / bulk-copy primitives (PTX, sm_90+; SASS: SYNCS.*, UBLKCP) ---------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
@@ -175,33 +179,40 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 
 // ---- the evaluation kernel -------------------------------------------------------------
 // One work item = (i-block ib, j-split sp): NT/JL i-particles against tiles [sp*tps, sp*tps+nt).
-// JLT = 1: one i per thread.  JLT = 0: JL (runtime, power of two <= 32) consecutive lanes share
-// one i and stride through the tile.  `tc` counts the tiles this CTA has consumed so far: ring
-// stage = tc & 1, mbarrier phase = (tc >> 1) & 1, so the ring carries over from item to item.
+// JL (compile time, a power of two <= 32) consecutive lanes share one i and stride through the tile:
+// JL = 1 is one i per thread (m >= NT); JL > 1 keeps all lanes busy when the active set is small
+// (the paper shrinks its thread blocks instead).  `tc` counts the tiles this CTA has
+// consumed so far: ring stage = tc & 1, mbarrier phase = (tc >> 1) & 1, so the ring carries over
+// from item to item.
 // MX: 0 = FP64, 1 = mixed precision (reading G27), 2 = FP64 acceleration and jerk only
 // The NT threads that work on an item are a whole CTA (VS = 0: tid = threadIdx.x, block barrier) or a
-// "virtual CTA" inside a larger one (the resident loop of nb_resident.cu): one warp (VS = 1, warp barrier)
-// or NT = 128 threads on the named barrier `bar_id` (VS = 2).  The arithmetic and its order are the same.
+// "virtual CTA" of NT threads on the named barrier `bar_id` inside a larger CTA (VS = 2, the resident
+// loop of nb_resident.cu).  The arithmetic and its order are the same.
+// Output: element (component c, slot k, split sp) goes to out[c * cstride + k * kstride + sp * sstride]
+// (PartLayout below).
 template <int VS>
 __device__ __forceinline__ void vcta_sync(const int bar_id, const int nthreads)
 {
     if (VS == 0) __syncthreads();
-    else if (VS == 1) __syncwarp();
     else asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "r"(nthreads) : "memory");
 }
 
-template <int NT, int TJ, int JLT, bool GUARD0, int MX, int UNR, int VS = 0>
+template <int NT, int TJ, int JL, bool GUARD0, int MX, int UNR, int VS = 0>
 __device__ __forceinline__ void force_item(const double *__restrict__ jp, const double *__restrict__ jstream,
                                            const int32_t *__restrict__ active, const int m, const int ib, const int sp, const int tiles_total,
-                                           const int tiles_per_split, const int JL, const double eps2,
-                                           double *__restrict__ out, const size_t cstride, const size_t sstride,
+                                           const int tiles_per_split, const double eps2,
+                                           double *__restrict__ out, const size_t cstride, const size_t kstride, const size_t sstride,
                                            double (*tile)[TJ * REC], uint64_t *full, unsigned &tc,
                                            const int tid_in = 0, const int bar_id = 0)
 {
+    static_assert(JL >= 1 && JL <= 32 && (JL & (JL - 1)) == 0, "lanes per i: a power of two within one warp");
     constexpr int NS = 2;
     constexpr uint32_t TILE_BYTES = TJ * REC * sizeof(double);
+    constexpr int PER = TJ / JL;                          // pairs per thread and tile
+    constexpr int UNRJ = JL == 1 ? UNR : (PER >= 24 ? 12 : PER);
+    constexpr int UNRM = PER >= 6 ? 6 : PER;
     const int tid = VS == 0 ? (int)threadIdx.x : tid_in;
-    const int slots = NT / JL;              // i-particles per CTA
+    constexpr int slots = NT / JL;          // i-particles per CTA
     const int k = ib * slots + tid / JL;    // slot in the active list
     const int jl = tid % JL;                // j-lane
     const int t0 = sp * tiles_per_split;
@@ -236,33 +247,21 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
         const unsigned sg = tc & 1u;
         mbar_wait(&full[sg], (tc >> 1) & 1u);
         if (!warp_idle) {
-            const double *q = tile[sg];
+            const double *q = tile[sg] + jl * REC;
             if (MX == 1) {
                 AccF A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
                 const float eps2f = (float)eps2;
-                if (JLT) {
-#pragma unroll 6
-                    for (int jj = 0; jj < TJ; ++jj)
-                        pair_body_mx<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2f, A);
-                } else {
-#pragma unroll 2
-                    for (int jj = jl; jj < TJ; jj += JL)
-                        pair_body_mx<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2f, A);
-                }
+#pragma unroll UNRM
+                for (int jj = 0; jj < PER; ++jj)
+                    pair_body_mx<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * (JL * REC), eps2f, A);
                 T.ax += (double)A.ax; T.ay += (double)A.ay; T.az += (double)A.az;
                 T.jx += (double)A.jx; T.jy += (double)A.jy; T.jz += (double)A.jz;
                 T.sx += (double)A.sx; T.sy += (double)A.sy; T.sz += (double)A.sz;
             } else {
                 Acc9 A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
-                if (JLT) {
-#pragma unroll UNR
-                    for (int jj = 0; jj < TJ; ++jj)
-                        pair_body<GUARD0, MX != 2>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
-                } else {
-#pragma unroll 2
-                    for (int jj = jl; jj < TJ; jj += JL)
-                        pair_body<GUARD0, MX != 2>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * REC, eps2, A);
-                }
+#pragma unroll UNRJ
+                for (int jj = 0; jj < PER; ++jj)
+                    NB_PAIR_BODY<GUARD0, MX != 2>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * (JL * REC), eps2, A);
                 T.ax += A.ax; T.ay += A.ay; T.az += A.az;
                 T.jx += A.jx; T.jy += A.jy; T.jz += A.jz;
                 T.sx += A.sx; T.sy += A.sy; T.sz += A.sz;
@@ -276,7 +275,8 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
         ++tc;
     }
 
-    if (!JLT) {  // fixed-order butterfly over the JL lanes that share this i
+    if (JL > 1) {  // fixed-order butterfly over the JL lanes that share this i
+#pragma unroll
         for (int off = JL >> 1; off > 0; off >>= 1) {
             T.ax += __shfl_xor_sync(0xffffffffu, T.ax, off);
             T.ay += __shfl_xor_sync(0xffffffffu, T.ay, off);
@@ -290,11 +290,80 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
         }
     }
     if (k < m && jl == 0) {
-        double *o = out + (size_t)sp * sstride + k;
+        double *o = out + (size_t)sp * sstride + (size_t)k * kstride;
         o[0 * cstride] = T.ax; o[1 * cstride] = T.ay; o[2 * cstride] = T.az;
         o[3 * cstride] = T.jx; o[4 * cstride] = T.jy; o[5 * cstride] = T.jz;
         o[6 * cstride] = T.sx; o[7 * cstride] = T.sy; o[8 * cstride] = T.sz;
     }
+}
+
+// force_item for a lane count known only at run time (the geometry rule chooses it from m)
+template <int NT, int TJ, bool GUARD0, int MX, int UNR, int VS = 0>
+__device__ __forceinline__ void force_item_jl(const int JL, const double *__restrict__ jp, const double *__restrict__ jstream,
+                                              const int32_t *__restrict__ active, const int m, const int ib, const int sp,
+                                              const int tiles_total, const int tiles_per_split, const double eps2,
+                                              double *__restrict__ out, const size_t cstride, const size_t kstride, const size_t sstride,
+                                              double (*tile)[TJ * REC], uint64_t *full, unsigned &tc, const int tid_in = 0,
+                                              const int bar_id = 0)
+{
+#define NB_ITEM(J) force_item<NT, TJ, J, GUARD0, MX, UNR, VS>(jp, jstream, active, m, ib, sp, tiles_total, tiles_per_split, eps2, \
+                                                              out, cstride, kstride, sstride, tile, full, tc, tid_in, bar_id)
+    switch (JL) {
+        case 1: NB_ITEM(1); break;
+        case 2: NB_ITEM(2); break;
+        case 4: NB_ITEM(4); break;
+        case 8: NB_ITEM(8); break;
+        case 16: NB_ITEM(16); break;
+        default: NB_ITEM(32); break;
+    }
+#undef NB_ITEM
+}
+
+// ---- where the split partials live, and their fixed-order sum (Table 1 row 4) ----
+// One split: the evaluation writes f1[c][k] directly.  2..31 splits: part[sp][c][k] (split-major, coalesced
+// along k for the many elements of a large set), summed by ONE thread per element in ascending split order.
+// >= 32 splits (small sets): part[c][k][sp] (split-minor: the S values of an element are consecutive), summed by
+// ONE warp per element: lane l adds the splits l, l + 32, ... in ascending order, then the xor butterfly
+// 16, 8, 4, 2, 1.  Every driver sums through these two functions, so all agree bit for bit.
+struct PartLayout {
+    size_t cstride, kstride, sstride;
+};
+__host__ __device__ inline PartLayout part_layout(const int S, const int mpad, const int64_t Npad)
+{
+    PartLayout L;
+    if (S <= 1) { L.cstride = (size_t)Npad; L.kstride = 1; L.sstride = 0; }
+    else if (S < 32) { L.cstride = (size_t)mpad; L.kstride = 1; L.sstride = 9 * (size_t)mpad; }
+    else { L.cstride = (size_t)mpad * S; L.kstride = (size_t)S; L.sstride = 1; }
+    return L;
+}
+__device__ __forceinline__ double sum_splits_thread(const double *__restrict__ p, const int S, const size_t sstride)
+{
+    double acc = 0.0;
+    for (int s = 0; s < S; ++s) acc += p[(size_t)s * sstride];
+    return acc;
+}
+__device__ __forceinline__ double sum_splits_warp(const double *__restrict__ p, const int S, const int lane)
+{
+    double acc = 0.0;
+#pragma unroll 4
+    for (int s = lane; s < S; s += 32) acc += p[s];
+    for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+    return acc;
+}
+
+// All nine components of slot k, by one warp (all 32 lanes call it): f1[c][k] <- fixed-order sum over the splits.
+__device__ __forceinline__ void reduce_one(const double *__restrict__ part, const int S, const PartLayout &L, const int k,
+                                           const int lane, double *__restrict__ f1, const int64_t Npad)
+{
+    if (S < 32) {
+        if (lane < 9) f1[lane * Npad + k] = sum_splits_thread(part + lane * L.cstride + (size_t)k * L.kstride, S, L.sstride);
+    } else {
+        for (int cc = 0; cc < 9; ++cc) {
+            const double acc = sum_splits_warp(part + cc * L.cstride + (size_t)k * L.kstride, S, lane);
+            if (lane == 0) f1[cc * Npad + k] = acc;
+        }
+    }
+    __syncwarp();
 }
 
 }  // namespace nb

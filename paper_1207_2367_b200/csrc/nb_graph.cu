@@ -4,9 +4,8 @@
 // indices in and forces out (Table 1 rows 1, 2, 6, 9), and for the smallest
 // blocks that overhead is most of the step.  Here the kernels of a step read
 // (t_next, m) and the evaluation geometry from a control block in device memory, so their launch
-// configurations are fixed and `graph_batch` consecutive block steps (five kernels each:
-// gather+predict, evaluation variant A, variant B, reduction, corrector) are captured ONCE per
-// context as a CUDA graph.  The host replays the graph and looks at the control block only
+// configurations are fixed and `graph_batch` consecutive block steps (three kernels each:
+// gather+predict, evaluation, split sums+corrector) are captured ONCE per context as a CUDA graph.  The host replays the graph and looks at the control block only
 // once per batch; steps past t_end (or past the requested count) find `done` set and return
 // without touching the state, so overshooting inside a batch is harmless.
 //

@@ -32,8 +32,11 @@ struct Sched {                 // device-written, host-read (pinned, mapped)
 // Launch geometry of one evaluation: which kernel variant, how many
 // lanes share one i (JL), how many j-splits (S) of how many tiles each (tps), how many i-blocks.
 struct ForceGeom {
-    int variant;  // 0: variant A (128 threads, one i per thread), 1: variant B (one warp per CTA)
-    int JL, S, tps, n_ib, mpad;
+    int JL;       // lanes of a warp that share one i (1: one i per thread; 2..32 when the set is small)
+    int S, tps;   // j-splits, tiles per split
+    int n_ib;     // i-blocks of NT_E / JL particles
+    int mpad;     // set size rounded up to 32 (row length of the split-major partial buffer)
+    int pad_;
 };
 
 // Control block of the device-resident block-step loop (nb_graph.cu): lives in device memory,
@@ -78,8 +81,8 @@ inline cudaError_t launch_chain(void (*kern)(KArgs...), dim3 grid, dim3 block, c
 }
 #endif
 
-constexpr int NT_A = 128, TJ_A = 128, MINB_A = 4;   // variant A: one i per thread, m >= 128
-constexpr int NT_B = 32, TJ_B = 64, MINB_B = 16;    // variant B: one warp per CTA, small m
+constexpr int NT_E = 128, TJ_E = 128, MINB_E = 4;   // evaluation CTA: 128 threads, j-tiles of 128 records, 4 CTAs per SM
+constexpr int JL_MAX = 32;                           // at most one warp shares one i
 constexpr int64_t L2_CHUNK_BYTES = 24 << 20;         // j-stream piece kept L2-resident across i-block waves
 constexpr int GEOM_CACHE_M = 4096;                   // the device loop remembers the geometry of set sizes up to this
 constexpr int MAX_WAVES = 64;                       // the split search considers 1..MAX_WAVES waves
@@ -124,35 +127,32 @@ __host__ __device__ inline int choose_split(const SplitProblem &p)
 
 // Geometry of the evaluation of m particles against Npad records, in two halves so that the
 // device can score the split candidates with one thread each (geom_finish takes the winner).
-__host__ __device__ inline SplitProblem geom_begin(ForceGeom &g, int64_t m, int64_t Npad, int n_sm, int occA, int occB,
+// Lanes per i: as many (a power of two, at most one warp) as keep m * JL within one CTA, so that a small
+// set still fills the lanes of its CTA; the j-splits then fill the machine.
+__host__ __device__ inline SplitProblem geom_begin(ForceGeom &g, int64_t m, int64_t Npad, int n_sm, int occ,
                                                    int64_t partials_cap, int force_jlanes)
 {
-    const bool varA = (m >= 128) && !(force_jlanes > 1);
     int JL = 1;
-    if (!varA) {
-        if (force_jlanes >= 1) JL = force_jlanes;
-        else { while (JL < 8 && m * (JL * 2) <= 32) JL *= 2; }
-    }
-    const int NT = varA ? NT_A : NT_B, TJ = varA ? TJ_A : TJ_B;
-    const int64_t slots_per_cta = NT / JL;
+    if (force_jlanes >= 1) JL = force_jlanes < JL_MAX ? force_jlanes : JL_MAX;
+    else { while (JL < JL_MAX && m * (JL * 2) <= NT_E) JL *= 2; }
+    const int64_t slots_per_cta = NT_E / JL;
     SplitProblem p;
     p.n_ib = (m + slots_per_cta - 1) / slots_per_cta;
-    p.tiles = Npad / TJ;
-    p.slots = (int64_t)n_sm * (varA ? occA : occB);
+    p.tiles = Npad / TJ_E;
+    p.slots = (int64_t)n_sm * occ;
     const int64_t mpad = (m + 31) & ~(int64_t)31;
     p.s_cap = partials_cap / (9 * mpad);
-    g.variant = varA ? 0 : 1; g.JL = JL; g.n_ib = (int)p.n_ib; g.mpad = (int)mpad;
+    g.JL = JL; g.n_ib = (int)p.n_ib; g.mpad = (int)mpad; g.pad_ = 0;
     return p;
 }
 __host__ __device__ inline void geom_finish(ForceGeom &g, const SplitProblem &p, int S_auto, int force_split)
 {
-    const int TJ = g.variant == 0 ? TJ_A : TJ_B;
     int S = force_split >= 1 ? (int)(force_split < p.tiles ? force_split : p.tiles) : S_auto;
     if (force_split < 1 && p.n_ib > p.slots) {
         // More than one wave of i-blocks re-reads the whole j-stream once per wave.  Keep the piece
         // that the concurrently running CTAs stream below L2_CHUNK_BYTES (a cyclic sweep over more
         // than the L2 of one die misses on every pass), when the partial sums fit.
-        const int64_t tps_max = L2_CHUNK_BYTES / ((int64_t)TJ * REC * 8);
+        const int64_t tps_max = L2_CHUNK_BYTES / ((int64_t)TJ_E * REC * 8);
         const int64_t s_min = (p.tiles + tps_max - 1) / tps_max;
         if (s_min > S && s_min <= p.s_cap) S = (int)s_min;
     }
@@ -161,11 +161,11 @@ __host__ __device__ inline void geom_finish(ForceGeom &g, const SplitProblem &p,
     S = (int)((p.tiles + tps - 1) / tps);
     g.S = S; g.tps = (int)tps;
 }
-__host__ __device__ inline ForceGeom choose_geom(int64_t m, int64_t Npad, int n_sm, int occA, int occB,
+__host__ __device__ inline ForceGeom choose_geom(int64_t m, int64_t Npad, int n_sm, int occ,
                                                  int64_t partials_cap, int force_split, int force_jlanes)
 {
     ForceGeom g;
-    const SplitProblem p = geom_begin(g, m, Npad, n_sm, occA, occB, partials_cap, force_jlanes);
+    const SplitProblem p = geom_begin(g, m, Npad, n_sm, occ, partials_cap, force_jlanes);
     geom_finish(g, p, force_split >= 1 ? 1 : choose_split(p), force_split);
     return g;
 }
@@ -226,7 +226,7 @@ struct nb_ctx {
     int64_t j_begin, j_end;         // j-shard evaluated by nb_force (nb_set_j_range); default [0, N)
     int precision;                  // 0: FP64 throughout (default); 1: the paper's mixed SP/DP pair arithmetic
     int64_t last_launch[5];
-    int occ[8];                     // resident CTAs per SM of each evaluation-kernel variant
+    int occ[8];                     // resident CTAs per SM: [0] k_force (the geometry rule uses it), [1] k_force_persistent
 
     // statistics
     int64_t n_steps;
@@ -247,7 +247,7 @@ namespace nb {
 int launch_force(nb_ctx *ctx, const int32_t *active, int64_t m, bool no_snap = false);
 int launch_check_indices(nb_ctx *ctx, const int32_t *idx, int64_t m);   // debug: fills ctx->h_dbg (after a sync)
 int query_force_occupancy(nb_ctx *ctx);
-int enqueue_force_persistent(nb_ctx *ctx);   // both variants + reduction; set size and geometry come from ctx->ctl
+int enqueue_force_persistent(nb_ctx *ctx);   // evaluation of the graph-driven loop; set size and geometry come from ctx->ctl
 // f1[c][k] -> out[q][k][3] (q = 0 acc, 1 jerk, 2 snap) contiguous in ctx->stage
 int launch_unpack_f1(nb_ctx *ctx, int64_t m);
 int launch_f1_contig(nb_ctx *ctx, int64_t m, double *buf, bool to_f1);
@@ -266,7 +266,7 @@ int launch_full_state(nb_ctx *ctx, double *state, bool to_ctx);
 int launch_tmax(nb_ctx *ctx);                                        // d_sched->t_next = max t_i
 
 int enqueue_graph_gather_predict(nb_ctx *ctx, int parity);           // active list + predictor of one step
-int enqueue_graph_correct(nb_ctx *ctx, int parity);           // corrector + bookkeeping
+int enqueue_graph_correct(nb_ctx *ctx, int parity);           // split sums + corrector + bookkeeping
 int launch_graph_begin(nb_ctx *ctx, double t_end, int64_t steps);    // seeds ctl (t_end, steps_left, tmin)
 
 // ----- nb_graph.cu

@@ -11,11 +11,11 @@
 //   phase 1  gather + predict   Table 1 row 1 + Eq. 3-7: one pass over the particles (as k_g_gather_predict)
 //   -- cluster barrier --
 //   phase 2  evaluate           the SAME items (i-block, j-split) of the SAME geometry rule as the other
-//                               drivers, each worked by a "virtual CTA" of this cluster (a warp for variant B,
-//                               128 threads on a named barrier for variant A) through force_item
+//                               drivers, each worked by a "virtual CTA" of this cluster (128 threads on a
+//                               named barrier) through force_item
 //   -- cluster barrier --
 //   phase 3  reduce + correct   one warp per active particle: the split partials in the fixed order of
-//                               k_reduce_thread / k_reduce_warp, then correct_one (Eq. 11-16) by lane 0
+//                               part_layout / sum_splits_*, then correct_one (Eq. 11-16) by lane 0
 //   -- cluster barrier --
 //
 // The state stays in global memory (L2-resident at these sizes); the predicted stream written in phase 1
@@ -32,17 +32,12 @@ namespace nb {
 
 constexpr int RES_THREADS = 512;                      // 16 warps per CTA: 4 per SM sub-partition
 constexpr int RES_WARPS = RES_THREADS / 32;
-constexpr int RES_VA = RES_THREADS / NT_A;            // virtual CTAs of variant A per CTA
+constexpr int RES_VC = RES_THREADS / NT_E;            // virtual evaluation CTAs per CTA
 constexpr int RES_GEOM_SLOTS = 64;                    // per-CTA direct-mapped memory of geometries by set size
 
 struct ResShared {
-    // tile rings: variant A uses RES_VA rings of 2 x TJ_A records, variant B RES_WARPS rings of 2 x TJ_B
-    union {
-        double a[RES_VA][2][TJ_A * REC];
-        double b[RES_WARPS][2][TJ_B * REC];
-    } tile;
-    uint64_t full_a[RES_VA][2];
-    uint64_t full_b[RES_WARPS][2];
+    double tile[RES_VC][2][TJ_E * REC];   // one two-stage ring of j-tiles per virtual CTA
+    uint64_t full[RES_VC][2];
     ForceGeom geom[RES_GEOM_SLOTS];
     int geom_m[RES_GEOM_SLOTS];
     SplitProblem sp;
@@ -76,13 +71,13 @@ __device__ __forceinline__ void res_block_min_to(double v, unsigned long long *d
 // The geometry of a set size, identical to choose_geom(): remembered per CTA (block-step runs see the same few
 // sizes again and again); on a miss the split candidates are scored by one thread each.  Called by all threads.
 __device__ __forceinline__ ForceGeom res_geometry(ResShared &sh, const int m, const int64_t Npad, const int n_sm,
-                                                  const int occA, const int occB, const int64_t partials_limit,
+                                                  const int occ, const int64_t partials_limit,
                                                   const int force_split, const int force_jlanes)
 {
     const int slot = m & (RES_GEOM_SLOTS - 1);
     __syncthreads();
     if (sh.geom_m[slot] != m) {
-        if (threadIdx.x == 0) sh.sp = geom_begin(sh.g, m, Npad, n_sm, occA, occB, partials_limit, force_jlanes);
+        if (threadIdx.x == 0) sh.sp = geom_begin(sh.g, m, Npad, n_sm, occ, partials_limit, force_jlanes);
         __syncthreads();
         if (threadIdx.x <= MAX_WAVES) {
             int S;
@@ -109,7 +104,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
     k_resident_loop(const int64_t N, const int64_t Npad, const double eps2, const double eta, const double dt_min,
                     const double dt_max, double *t, double *dt, double *mass, double *r, double *v, double *a,
                     double *j, double *s, double *c, double *jp, int32_t *active_list, double *f1, double *partials,
-                    StepCtl *ctl, const int n_sm, const int occA, const int occB, const int64_t partials_limit,
+                    StepCtl *ctl, const int n_sm, const int occ, const int64_t partials_limit,
                     const int force_split, const int force_jlanes)
 {
     extern __shared__ __align__(128) unsigned char res_smem[];
@@ -120,20 +115,27 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
     const double inf = __longlong_as_double(0x7ff0000000000000LL);
 
     if (tid == 0) {
-        for (int q = 0; q < RES_VA; ++q) { mbar_init(&sh.full_a[q][0], 1); mbar_init(&sh.full_a[q][1], 1); }
-        for (int q = 0; q < RES_WARPS; ++q) { mbar_init(&sh.full_b[q][0], 1); mbar_init(&sh.full_b[q][1], 1); }
+        for (int q = 0; q < RES_VC; ++q) { mbar_init(&sh.full[q][0], 1); mbar_init(&sh.full[q][1], 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int q = tid; q < RES_GEOM_SLOTS; q += RES_THREADS) sh.geom_m[q] = -1;
     __syncthreads();
-    unsigned tc_a = 0, tc_b = 0;    // tiles consumed so far through this thread's variant-A / variant-B ring
+    unsigned tc = 0;                // tiles consumed so far through this thread's ring
     volatile StepCtl *vctl = ctl;
+#ifdef NB_RES_TIMING   // development aid: cycles per phase of the step, summed by one thread into unused histogram bins
+    long long tph[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    long long tq = clock64();
+#define NB_TICK(q) do { const long long now_ = clock64(); tph[q] += now_ - tq; tq = now_; } while (0)
+#else
+#define NB_TICK(q) do { } while (0)
+#endif
 
     for (int p = 0;; p ^= 1) {
         // ---- phase 1: gather + predict.  Every thread of the cluster evaluates the same condition from
         // values that nothing modifies before the second barrier of the step.
         const double tn = __longlong_as_double((long long)vctl->tmin[p]);
         if (vctl->steps_left <= 0 || !(tn <= vctl->t_end)) break;
+        NB_TICK(0);
         double vmin = inf;
         for (int64_t base = (int64_t)gwarp * 32; base < N; base += (int64_t)gwarps * 32) {   // warp-uniform trip count
             const int64_t i = base + lane;
@@ -155,58 +157,37 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
             }
         }
         res_block_min_to(vmin, &ctl->tmin[1 - p], sh.red);
+        NB_TICK(1);
         fence_proxy_async();          // the records just stored are read by bulk copies (async proxy) below
         cluster_sync_all();
         fence_proxy_async();
+        NB_TICK(2);
 
         // ---- phase 2: evaluate
         const int m = vctl->cnt[p];
-        const ForceGeom g = res_geometry(sh, m, Npad, n_sm, occA, occB, partials_limit, force_split, force_jlanes);
+        const ForceGeom g = res_geometry(sh, m, Npad, n_sm, occ, partials_limit, force_split, force_jlanes);
+        NB_TICK(3);
         const int32_t *active = (m == N) ? nullptr : active_list;
         double *out = g.S > 1 ? partials : f1;
-        const size_t cstride = g.S > 1 ? (size_t)g.mpad : (size_t)Npad;
-        const size_t sstride = 9 * (size_t)g.mpad;
+        const PartLayout L = part_layout(g.S, g.mpad, Npad);
         const long long items = (long long)g.n_ib * g.S;
-        if (g.variant == 0) {
-            const int vc = tid / NT_A, vt = tid % NT_A;        // virtual CTA of 128 threads, named barrier 1 + vc
-            const int tiles_total = (int)(Npad / TJ_A);
-            for (long long w = (long long)rank * RES_VA + vc; w < items; w += (long long)n_cta * RES_VA)
-                force_item<NT_A, TJ_A, 1, GUARD0, MX, 12, 2>(jp, jp, active, m, (int)(w % g.n_ib), (int)(w / g.n_ib), tiles_total,
-                                                          g.tps, 1, eps2, out, cstride, sstride, sh.tile.a[vc], sh.full_a[vc],
-                                                          tc_a, vt, 1 + vc);
-        } else {
-            const int tiles_total = (int)(Npad / TJ_B);        // virtual CTA = this warp
-            for (long long w = gwarp; w < items; w += gwarps)
-                force_item<NT_B, TJ_B, 0, GUARD0, MX, 12, 1>(jp, jp, active, m, (int)(w % g.n_ib), (int)(w / g.n_ib), tiles_total,
-                                                          g.tps, g.JL, eps2, out, cstride, sstride, sh.tile.b[warp],
-                                                          sh.full_b[warp], tc_b, lane, 0);
+        {
+            const int vc = tid / NT_E, vt = tid % NT_E;        // virtual CTA of 128 threads, named barrier 1 + vc
+            const int tiles_total = (int)(Npad / TJ_E);
+            for (long long w = (long long)rank * RES_VC + vc; w < items; w += (long long)n_cta * RES_VC)
+                force_item_jl<NT_E, TJ_E, GUARD0, MX, 12, 2>(g.JL, jp, jp, active, m, (int)(w % g.n_ib), (int)(w / g.n_ib),
+                                                             tiles_total, g.tps, eps2, out, L.cstride, L.kstride, L.sstride,
+                                                             sh.tile[vc], sh.full[vc], tc, vt, 1 + vc);
         }
+        NB_TICK(4);
         cluster_sync_all();
+        NB_TICK(5);
 
-        // ---- phase 3: reduce + correct, one warp per active particle.  The sum over the splits runs in the
-        // order of k_reduce_thread (S < 32: ascending, one thread per component) or k_reduce_warp (lane-strided,
-        // then the xor butterfly), so that all drivers agree bit for bit.
+        // ---- phase 3: reduce + correct, one warp per active particle; the sum over the splits runs in the
+        // order every driver uses (part_layout, sum_splits_*), so that all agree bit for bit.
         vmin = inf;
         for (int k = gwarp; k < m; k += gwarps) {
-            if (g.S > 1) {
-                if (g.S < 32) {
-                    if (lane < 9) {
-                        const double *pp = partials + lane * cstride + k;
-                        double acc = 0.0;
-                        for (int sp = 0; sp < g.S; ++sp) acc += pp[(size_t)sp * sstride];
-                        f1[lane * Npad + k] = acc;
-                    }
-                } else {
-                    for (int cc = 0; cc < 9; ++cc) {
-                        const double *pp = partials + cc * cstride + k;
-                        double acc = 0.0;
-                        for (int sp = lane; sp < g.S; sp += 32) acc += pp[(size_t)sp * sstride];
-                        for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
-                        if (lane == 0) f1[cc * Npad + k] = acc;
-                    }
-                }
-                __syncwarp();
-            }
+            if (g.S > 1) reduce_one(partials, g.S, L, k, lane, f1, Npad);
             if (lane == 0) {
                 const int64_t i = active ? active[k] : k;
                 vmin = fmin(vmin, correct_one(k, i, Npad, tn, eta, dt_min, dt_max, f1, t, dt, r, v, a, j, s, c));
@@ -226,8 +207,14 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
             ctl->tmin[p] = 0x7ff0000000000000ULL;   // consumed: slot p collects the minimum of the step after next
             ctl->cnt[p] = 0;
         }
+        NB_TICK(6);
         cluster_sync_all();
+        NB_TICK(7);
     }
+#ifdef NB_RES_TIMING
+    if (rank == 0 && tid == 0)
+        for (int q = 0; q < 8; ++q) ctl->hist[40 + q] += tph[q];
+#endif
     if (rank == 0 && tid == 0) ctl->done = 1;
 }
 
@@ -255,7 +242,7 @@ static cudaError_t launch_resident(nb_ctx *ctx, int n_cta)
     if (n_clusters < 1) return cudaErrorLaunchOutOfResources;
     return cudaLaunchKernelEx(&cfg, kern, ctx->N, ctx->Npad, ctx->eps2, ctx->eta, ctx->dt_min, ctx->dt_max, ctx->t, ctx->dt,
                               ctx->mass, ctx->r, ctx->v, ctx->a, ctx->j, ctx->s, ctx->c, ctx->jp, ctx->active, ctx->f1,
-                              ctx->partials, ctx->ctl, ctx->n_sm, ctx->occ[0], ctx->occ[1], (int64_t)ctx->partials_limit,
+                              ctx->partials, ctx->ctl, ctx->n_sm, ctx->occ[0], (int64_t)ctx->partials_limit,
                               ctx->force_split, ctx->force_jlanes);
 }
 

@@ -6,6 +6,7 @@
 //   start-up             DESIGN.md reading G8            k_startup_commit
 // All of them stream the SoA state once; they are HBM- or latency-bound.
 #include "nb_internal.cuh"
+#include "nb_force_dev.cuh"
 #include "nb_step_dev.cuh"
 
 namespace nb {
@@ -456,8 +457,8 @@ __global__ void __launch_bounds__(SCHED_THREADS)
                        const double *__restrict__ dt, int32_t *__restrict__ active, StepCtl *__restrict__ ctl,
                        const double *__restrict__ mass, const double *__restrict__ r, const double *__restrict__ v,
                        const double *__restrict__ a, const double *__restrict__ j, const double *__restrict__ s,
-                       const double *__restrict__ c, double *__restrict__ jp, const int n_sm, const int occA,
-                       const int occB, const int64_t partials_limit, const int force_split, const int force_jlanes,
+                       const double *__restrict__ c, double *__restrict__ jp, const int n_sm, const int occ,
+                       const int64_t partials_limit, const int force_split, const int force_jlanes,
                        ForceGeom *__restrict__ geom_cache)
 {
     pdl_trigger();
@@ -520,7 +521,7 @@ __global__ void __launch_bounds__(SCHED_THREADS)
     }
     if (threadIdx.x == 0) {
         ctl->ticket = 0;
-        sp = geom_begin(sg, m, Npad, n_sm, occA, occB, partials_limit, force_jlanes);
+        sp = geom_begin(sg, m, Npad, n_sm, occ, partials_limit, force_jlanes);
     }
     __syncthreads();
     if (threadIdx.x <= MAX_WAVES) {
@@ -541,13 +542,16 @@ __global__ void __launch_bounds__(SCHED_THREADS)
     }
 }
 
-// Corrector and new dt for the active set (grid-stride over its slots), their share of the next
-// minimum, and -- block 0 -- the bookkeeping of the step; that touches only fields which no block of
-// this kernel reads (they read t_next, n_active, g, which the earlier kernels of the step published).
+// Sum of the split partials, corrector and new dt for the active set, their share of the next minimum,
+// and -- block 0 -- the bookkeeping of the step; that touches only fields which no block of this kernel
+// reads (they read t_next, n_active, g, which the earlier kernels of the step published).
+// One split: the evaluation wrote f1 itself, one thread corrects one particle.  Several splits: one WARP
+// per active particle sums its nine components in the fixed order of part_layout / sum_splits_* (the order
+// of k_reduce_thread / k_reduce_warp of the host-issued path), stores them to f1, and lane 0 corrects.
 __global__ void __launch_bounds__(SCHED_THREADS)
-    k_g_correct(const int p, const int64_t N, const int64_t Npad, const int32_t *__restrict__ active_list,
+    k_g_reduce_correct(const int p, const int64_t N, const int64_t Npad, const int32_t *__restrict__ active_list,
                        StepCtl *__restrict__ ctl, const double eta, const double dt_min, const double dt_max,
-                       const double *__restrict__ f1, double *__restrict__ ti,
+                       const double *__restrict__ partials, double *__restrict__ f1, double *__restrict__ ti,
                        double *__restrict__ dti, double *__restrict__ r, double *__restrict__ v,
                        double *__restrict__ a, double *__restrict__ j, double *__restrict__ s, double *__restrict__ c)
 {
@@ -556,11 +560,25 @@ __global__ void __launch_bounds__(SCHED_THREADS)
     if (ctl->done) return;
     const int m = (int)ctl->n_active;
     const double tn = ctl->t_next;
+    const int S = ctl->g.S;
     const int32_t *active = (m == N) ? nullptr : active_list;
     double vmin = __longlong_as_double(0x7ff0000000000000LL);
-    for (int k = blockIdx.x * SCHED_THREADS + threadIdx.x; k < m; k += gridDim.x * SCHED_THREADS) {
-        const int64_t i = active ? active[k] : k;
-        vmin = fmin(vmin, correct_one(k, i, Npad, tn, eta, dt_min, dt_max, f1, ti, dti, r, v, a, j, s, c));
+    if (S <= 1) {
+        for (int k = blockIdx.x * SCHED_THREADS + threadIdx.x; k < m; k += gridDim.x * SCHED_THREADS) {
+            const int64_t i = active ? active[k] : k;
+            vmin = fmin(vmin, correct_one(k, i, Npad, tn, eta, dt_min, dt_max, f1, ti, dti, r, v, a, j, s, c));
+        }
+    } else {
+        const PartLayout L = part_layout(S, ctl->g.mpad, Npad);
+        const int lane = threadIdx.x & 31;
+        const int nwarps = (gridDim.x * SCHED_THREADS) >> 5;
+        for (int k = (blockIdx.x * SCHED_THREADS + threadIdx.x) >> 5; k < m; k += nwarps) {
+            reduce_one(partials, S, L, k, lane, f1, Npad);
+            if (lane == 0) {
+                const int64_t i = active ? active[k] : k;
+                vmin = fmin(vmin, correct_one(k, i, Npad, tn, eta, dt_min, dt_max, f1, ti, dti, r, v, a, j, s, c));
+            }
+        }
     }
     block_min_to(vmin, &ctl->tmin[1 - p]);
     if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -593,7 +611,7 @@ int enqueue_graph_gather_predict(nb_ctx *ctx, int parity)
     const unsigned np = (unsigned)((ctx->N + SCHED_THREADS - 1) / SCHED_THREADS);
     launch_chain(k_g_gather_predict, dim3(np), dim3(SCHED_THREADS), ctx->stream, ctx->use_graph == 2, parity, ctx->N,
                  ctx->Npad, ctx->t, ctx->dt, ctx->active, ctx->ctl, ctx->mass, ctx->r, ctx->v, ctx->a, ctx->j, ctx->s,
-                 ctx->c, ctx->jp, ctx->n_sm, ctx->occ[0], ctx->occ[1], (int64_t)ctx->partials_limit, ctx->force_split,
+                 ctx->c, ctx->jp, ctx->n_sm, ctx->occ[0], (int64_t)ctx->partials_limit, ctx->force_split,
                  ctx->force_jlanes, ctx->geom_cache);
     NB_LAUNCH_CHECK(ctx, "k_g_gather_predict");
     return NB_OK;
@@ -601,12 +619,13 @@ int enqueue_graph_gather_predict(nb_ctx *ctx, int parity)
 
 int enqueue_graph_correct(nb_ctx *ctx, int parity)
 {
+    // enough warps for one per active particle of a small set; large sets (one split) go thread per particle
     int64_t g = (ctx->N + SCHED_THREADS - 1) / SCHED_THREADS;
     if (g > 4 * ctx->n_sm) g = 4 * ctx->n_sm;
-    launch_chain(k_g_correct, dim3((unsigned)g), dim3(SCHED_THREADS), ctx->stream, ctx->use_graph == 2, parity, ctx->N,
-                 ctx->Npad, ctx->active, ctx->ctl, ctx->eta, ctx->dt_min, ctx->dt_max, ctx->f1, ctx->t, ctx->dt, ctx->r,
-                 ctx->v, ctx->a, ctx->j, ctx->s, ctx->c);
-    NB_LAUNCH_CHECK(ctx, "k_g_correct");
+    launch_chain(k_g_reduce_correct, dim3((unsigned)g), dim3(SCHED_THREADS), ctx->stream, ctx->use_graph == 2, parity, ctx->N,
+                 ctx->Npad, ctx->active, ctx->ctl, ctx->eta, ctx->dt_min, ctx->dt_max, ctx->partials, ctx->f1, ctx->t, ctx->dt,
+                 ctx->r, ctx->v, ctx->a, ctx->j, ctx->s, ctx->c);
+    NB_LAUNCH_CHECK(ctx, "k_g_reduce_correct");
     return NB_OK;
 }
 

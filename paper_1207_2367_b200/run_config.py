@@ -210,7 +210,7 @@ def main():
     ap.add_argument("--ns", default=None, help="comma-separated N list for --experiment fig1")
     ap.add_argument("--ms", default=None, help="comma-separated active-set sizes for --config 4 (default: the config's five)")
     ap.add_argument("--heavy-frac", type=float, default=0.05)
-    ap.add_argument("--loop", type=int, default=None, choices=[0, 1, 2], help="0: host-driven loop, 1: device-driven graph batches (default), 2: the same with programmatic dependent launch")
+    ap.add_argument("--loop", type=int, default=None, choices=[0, 1, 2, 3], help="0: host-driven loop, 1: device-driven graph batches, 2: the same with programmatic dependent launch, 3: cluster-resident loop (N <= 16384); default: 3 for N <= 2048, else 1")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"],
                     help="evaluation arithmetic: fp64 (default) or the paper's mixed SP/DP scheme (PAPER.md:287)")
     a = ap.parse_args()
@@ -239,7 +239,7 @@ def main():
         N = a.n or c["N"]
         steps = a.steps if a.steps is not None else c.get("n_block_steps")
         out = run_integration(nb, a.config, c, N, a.t_end if a.t_end is not None else c.get("t_end"), steps, a.loop)
-        out["loop"] = "host" if a.loop == 0 else "device"
+        out["loop"] = {None: "default", 0: "host", 1: "graph", 2: "graph+pdl", 3: "resident"}[a.loop]
     elif a.config == 3:
         Ns = [a.n] if a.n else [n for n in c["N"] if not a.max_n or n <= a.max_n]
         out = run_force(nb, 3, c, Ns, None)
