@@ -209,10 +209,13 @@ int nb_set_debug(nb_ctx *ctx, int on);
  *   1  device-driven CUDA-graph batches (kernels read (t_next, n_active) from device memory);
  *   2  the same graph with its kernels chained by programmatic dependent launch (measured slower than
  *      plain graph edges on B200, kept for comparison);
- *   3  ONE kernel resident on one thread-block cluster runs every step, its phases separated by the
- *      hardware cluster barrier instead of kernel boundaries (no host round trip and no launch per step;
- *      the small blocks); at most 16 SMs work, so it serves N <= 16384 (NB_EINVAL above).
- * Default: 3 for N <= 2048, else 1.  nb_run_steps with a per-step log always uses 0.          */
+ *   3  ONE kernel resident on one thread-block cluster (up to 16 SMs) keeps the whole system in shared
+ *      memory and runs every step, its phases separated by the hardware cluster barrier: no launch, no host
+ *      round trip and no trip to L2 per step (the small blocks).  Serves N <= 2048 (NB_EINVAL
+ *      above).  It adds the pair terms of a particle in its own fixed order (per owner CTA, then over the CTAs),
+ *      so its results agree with modes 0-2 to rounding, not bit for bit (any order is correct, G18).
+ * Modes 0, 1, 2 give bit-identical states.  Default: 3 for N <= 2048, else 1.  nb_run_steps with a per-step
+ * log always uses 0.                                                                         */
 int nb_set_loop_mode(nb_ctx *ctx, int device_driven);
 
 /* What the last nb_force launched: out [host] = {threads per CTA, j-lanes per i, j-splits,

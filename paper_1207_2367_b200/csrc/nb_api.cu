@@ -140,6 +140,7 @@ extern "C" int nb_init(nb_ctx **out, int64_t N, const double *pos, const double 
     if (cudaHostAlloc((void **)&ctx->h_ctl, sizeof(StepCtl), cudaHostAllocDefault) != cudaSuccess) return fail(NB_ENOMEM);
     memset(ctx->h_ctl, 0, sizeof(StepCtl));
     ctx->use_graph = N <= RES_AUTO_N ? 3 : 1;
+    ctx->loop_auto = true;
     ctx->j_begin = 0; ctx->j_end = N;
     if ((rc = query_force_occupancy(ctx))) return fail(rc);
 
@@ -528,6 +529,7 @@ extern "C" int nb_set_loop_mode(nb_ctx *ctx, int device_driven)
     if (device_driven == 3 && ctx->N > RES_MAX_N)
         return set_err(ctx, NB_EINVAL, "nb_set_loop_mode: mode 3 (cluster-resident loop) serves N <= %lld", (long long)RES_MAX_N);
     ctx->use_graph = device_driven;
+    ctx->loop_auto = false;
     return NB_OK;
 }
 

@@ -19,13 +19,35 @@ __device__ __forceinline__ double rsqrt_seed(double s)
     return y;
 }
 
-// One pair interaction, Eq. 8-10 in the factored form (DESIGN.md section 6):
-//   s = |dr|^2 + eps^2, w = m_j s^(-3/2), g = -3 (dr.dv)/s, b3 = -3 beta,
-//   u = dv + g dr,  A0 = w dr,  A1 = w u,  A2 = w (da + 2 g u + b3 dr).
+// One pair interaction, Eq. 8-10 in the factored form (DESIGN.md section 6.1):
+//   s = |dr|^2 + eps^2,  y = s^(-1/2),  alpha = (dr.dv)/s,  beta = (|dv|^2 + dr.da)/s + alpha^2,
+//   u = dv - 3 alpha dr,  A0 = w dr,  A1 = w u,  A2 = w (da - 6 alpha u - 3 beta dr),  w = m_j s^(-3/2).
 // q points at the packed record {x y z vx vy vz ax ay az m} of particle j in shared memory.
-// SNAP = false (start-up pass 1, G8: only a and jerk are wanted; the snap of that pass would be
-// discarded): the a_ij differences, r.a, beta and the snap accumulation are left out -- 31 instead
-// of 53 FP64 instructions; a and jerk are computed by the same expressions.
+//
+// 51 FP64-pipe instructions (32 DFMA + 10 DMUL + 9 DADD) and one MUFU.RSQ64H:
+//   * the factor 3 of "3 alpha", "3 beta" rides on the inverse square root: the Newton step produces
+//     y' = sqrt(3) y (its three constants carry the sqrt(3)), so ri2 = y'^2 = 3/s, g = ri2 (dr.dv) = 3 alpha and
+//     b3 = ri2 (|dv|^2 + dr.da) + g^2/3 = 3 beta come out directly and enter the FMAs negated (operand
+//     modifiers are free);  w' = m_j y' ri2 = 3 sqrt(3) w, so the accumulators hold 3 sqrt(3) times the sums
+//     and the caller scales them ONCE per item by PAIR_SCALE = 1/(3 sqrt(3)) (force_item);
+//   * 2 g is an increment of the exponent field (integer pipe, exact for every normal g; g = 0 or
+//     subnormal gives a value below 4.5e-308 whose product with u is far below one ulp of anything here).
+// The statement ORDER below is not cosmetic.  The FP64 datapath reads one fresh 64-bit operand per cycle
+// and SM sub-partition, so an instruction with three distinct register sources costs 3 cycles instead of 2
+// unless one of them sits in the operand-reuse cache, i.e. the preceding FP64 instruction of the same warp
+// read it in the same operand slot.  ptxas -O1 (this file's setting, _build.py)
+// keeps close to the order written here; this order (found by a randomised search over dependency-respecting
+// orders and operand orders, scored on the SASS by sum of max(2, fresh operands)) has 107 cycles of
+// operand fetch per pair against 102 for the 51 instructions alone; the round-1 body had 124.
+// SNAP = false (start-up pass 1, G8: only a and jerk are wanted): everything that only feeds the snap is
+// dead code in that instantiation -- 29 FP64 instructions; a and jerk are computed by the same expressions.
+constexpr double PAIR_SCALE = 0.19245008972987526;   // 1 / (3 sqrt(3))
+
+__device__ __forceinline__ double twice(const double g)
+{
+    return __hiloint2double(__double2hiint(g) + 0x00100000, __double2loint(g));
+}
+
 template <bool GUARD0, bool SNAP = true>
 __device__ __forceinline__ void pair_body(const double xi, const double yi, const double zi,
                                           const double vxi, const double vyi, const double vzi,
@@ -37,58 +59,64 @@ __device__ __forceinline__ void pair_body(const double xi, const double yi, cons
     const double2 p2 = *reinterpret_cast<const double2 *>(q + 4);
     const double2 p3 = *reinterpret_cast<const double2 *>(q + 6);
     const double2 p4 = *reinterpret_cast<const double2 *>(q + 8);
-    // differences and the three dot products, component by component (z, y, x)
-    const double dvz = p2.y - vzi, dvy = p2.x - vyi, dvx = p1.y - vxi;
-    double vr = dvz * dvz;
-    vr = fma(dvy, dvy, vr);
-    vr = fma(dvx, dvx, vr);
-    const double dz = p1.x - zi, daz = p4.x - azi;
-    double s = fma(dz, dz, eps2);
-    double rv = dz * dvz;
-    vr = fma(dz, daz, vr);
-    const double dy = p0.y - yi, day = p3.y - ayi;
-    s = fma(dy, dy, s);
-    rv = fma(dy, dvy, rv);
-    vr = fma(dy, day, vr);
-    const double dx = p0.x - xi, dax = p3.x - axi;
-    s = fma(dx, dx, s);
-    rv = fma(dx, dvx, rv);
-    vr = fma(dx, dax, vr);
     const double mj = p4.y;
+    const double dy = p0.y - yi;
+    const double dz = p1.x - zi;
+    const double s0 = fma(dy, dy, eps2);
+    const double dvz = p2.y - vzi;
+    const double dvx = p1.y - vxi;
+    const double daz = p4.x - azi;
+    const double vr0 = dz * daz;
+    const double dvy = p2.x - vyi;
+    const double dax = p3.x - axi;
+    const double dx = p0.x - xi;
+    const double s1 = fma(dx, dx, s0);
+    const double day = p3.y - ayi;
+    const double s = fma(dz, dz, s1);                 // |dr|^2 + eps^2
+    const double rv0 = dvy * dy;
+    const double vr1 = fma(dy, day, vr0);
+    const double vr2 = fma(dax, dx, vr1);
+    const double rv1 = fma(dx, dvx, rv0);
+    const double vr3 = fma(dvz, dvz, vr2);
     double y0 = rsqrt_seed(s);
     if (GUARD0) {  // eps = 0: a coincident pair (the self term) contributes nothing (G12)
         if ((__double2hiint(s) | __double2loint(s)) == 0) y0 = 0.0;
     }
-    // y = y0 (1 + e (1/2 + 3/8 e)), e = 1 - s y0^2: every instruction reads at most two registers
+    const double rv = fma(dz, dvz, rv1);              // dr.dv
+    const double vr4 = fma(dvx, dvx, vr3);
+    const double vr = fma(dvy, dvy, vr4);             // |dv|^2 + dr.da
+    // y' = sqrt(3) y0 (1 + e (1/2 + 3/8 e)), e = 1 - s y0^2: one third-order step on the 2^-21 seed
     const double y2 = y0 * y0;
     const double e = fma(-s, y2, 1.0);
-    const double p = fma(e, 0.375, 0.5);
-    const double ep1 = fma(e, p, 1.0);
-    const double y = y0 * ep1;         // s^(-1/2)
-    const double ri2 = y * y;          // 1/s
-    const double my = mj * y;
-    const double qq = ri2 * -3.0;
-    const double w = my * ri2;         // m_j s^(-3/2)
-    const double g = rv * qq;          // -3 alpha
-    const double qv = qq * vr;
+    const double p = fma(e, 0.649519052838329, 0.8660254037844386);      // sqrt(3) (3/8 e + 1/2)
+    const double ep1 = fma(e, p, 1.7320508075688772);                    // sqrt(3) (1 + e (...))
+    const double y = y0 * ep1;                        // sqrt(3) s^(-1/2)
+    const double ri2 = y * y;                         // 3 / s
+    const double g = ri2 * rv;                        // 3 alpha
     const double gg = g * g;
-    const double g2 = g + g;
-    const double b3 = fma(gg, -1.0 / 3.0, qv);  // -3 beta = -3 (v^2 + r.a)/s - 3 alpha^2
-    const double ux = fma(g, dx, dvx), uy = fma(g, dy, dvy), uz = fma(g, dz, dvz);
-    A.ax = fma(w, dx, A.ax);
-    A.ay = fma(w, dy, A.ay);
+    const double qv = ri2 * vr;
+    const double my = mj * y;
+    const double uy = fma(dy, -g, dvy);               // u = dv - 3 alpha dr
+    const double uz = fma(dz, -g, dvz);
+    const double b3 = fma(gg, 1.0 / 3.0, qv);         // 3 beta
+    const double t1y = fma(-b3, dy, day);
+    const double ux = fma(-g, dx, dvx);
+    const double g2 = twice(g);                       // 6 alpha
+    const double t1x = fma(-b3, dx, dax);
+    const double t1z = fma(dz, -b3, daz);
+    const double ty = fma(uy, -g2, t1y);              // t = da - 6 alpha u - 3 beta dr
+    const double tx = fma(ux, -g2, t1x);
+    const double tz = fma(-g2, uz, t1z);
+    const double w = ri2 * my;                        // 3 sqrt(3) m_j s^(-3/2)
+    if (SNAP) A.sy = fma(w, ty, A.sy);
     A.az = fma(w, dz, A.az);
-    A.jx = fma(w, ux, A.jx);
-    A.jy = fma(w, uy, A.jy);
+    if (SNAP) A.sz = fma(w, tz, A.sz);
+    A.ay = fma(dy, w, A.ay);
     A.jz = fma(w, uz, A.jz);
-    if (!SNAP) return;  // everything that only feeds the snap above is dead code in this instantiation
-    double tx = fma(g2, ux, dax), ty = fma(g2, uy, day), tz = fma(g2, uz, daz);
-    tx = fma(b3, dx, tx);
-    ty = fma(b3, dy, ty);
-    tz = fma(b3, dz, tz);
-    A.sx = fma(w, tx, A.sx);
-    A.sy = fma(w, ty, A.sy);
-    A.sz = fma(w, tz, A.sz);
+    A.jx = fma(ux, w, A.jx);
+    A.ax = fma(dx, w, A.ax);
+    A.jy = fma(uy, w, A.jy);
+    if (SNAP) A.sx = fma(w, tx, A.sx);
 }
 
 // The same pair in the paper's mixed precision (reading G27): the nine
@@ -135,10 +163,6 @@ __device__ __forceinline__ void pair_body_mx(const double xi, const double yi, c
     tx = fmaf(b3, dx, tx); ty = fmaf(b3, dy, ty); tz = fmaf(b3, dz, tz);
     A.sx = fmaf(w, tx, A.sx); A.sy = fmaf(w, ty, A.sy); A.sz = fmaf(w, tz, A.sz);
 }
-
-#ifndef NB_PAIR_BODY
-#define NB_PAIR_BODY pair_body
-#endif
 
 // ---- mbarrier / bulk-copy primitives (PTX, sm_90+; SASS: SYNCS.*, UBLKCP) ---------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
@@ -261,7 +285,7 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
                 Acc9 A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
 #pragma unroll UNRJ
                 for (int jj = 0; jj < PER; ++jj)
-                    NB_PAIR_BODY<GUARD0, MX != 2>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * (JL * REC), eps2, A);
+                    pair_body<GUARD0, MX != 2>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * (JL * REC), eps2, A);
                 T.ax += A.ax; T.ay += A.ay; T.az += A.az;
                 T.jx += A.jx; T.jy += A.jy; T.jz += A.jz;
                 T.sx += A.sx; T.sy += A.sy; T.sz += A.sz;
@@ -275,6 +299,11 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
         ++tc;
     }
 
+    if (MX != 1) {  // the FP64 pair body accumulates 3 sqrt(3) times the sums (pair_body)
+        T.ax *= PAIR_SCALE; T.ay *= PAIR_SCALE; T.az *= PAIR_SCALE;
+        T.jx *= PAIR_SCALE; T.jy *= PAIR_SCALE; T.jz *= PAIR_SCALE;
+        T.sx *= PAIR_SCALE; T.sy *= PAIR_SCALE; T.sz *= PAIR_SCALE;
+    }
     if (JL > 1) {  // fixed-order butterfly over the JL lanes that share this i
 #pragma unroll
         for (int off = JL >> 1; off > 0; off >>= 1) {

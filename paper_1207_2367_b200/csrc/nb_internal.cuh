@@ -86,7 +86,7 @@ constexpr int JL_MAX = 32;                           // at most one warp shares 
 constexpr int64_t L2_CHUNK_BYTES = 24 << 20;         // j-stream piece kept L2-resident across i-block waves
 constexpr int GEOM_CACHE_M = 4096;                   // the device loop remembers the geometry of set sizes up to this
 constexpr int MAX_WAVES = 64;                       // the split search considers 1..MAX_WAVES waves
-constexpr int64_t RES_MAX_N = 16384;                 // the cluster-resident loop (nb_resident.cu) serves N up to this
+constexpr int64_t RES_MAX_N = 2048;                  // the cluster-resident loop (nb_resident.cu) keeps N up to this on chip
 constexpr int64_t RES_AUTO_N = 2048;                 // ... and is the default driver up to this
 
 // Number of j-splits.  All CTAs do the same work per tile, so the cost of a launch is
@@ -219,6 +219,7 @@ struct nb_ctx {
     int64_t launches_per_batch;     // kernels in one replay of step_graph
     int use_graph;                  // loop mode: 0 host-issued calls; 1, 2 graph batches (2: with PDL); 3 cluster-resident loop
     int res_cluster;                // CTAs of the resident loop's cluster (16, or 8 where 16 cannot be scheduled)
+    bool loop_auto;                 // the loop mode is the default for this N (not set by nb_set_loop_mode)
     int graph_pdl;                  // the captured graph uses programmatic dependent launch
 
     // tuning

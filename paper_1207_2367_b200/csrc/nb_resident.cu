@@ -1,128 +1,241 @@
-// nb_resident.cu -- the block-step loop resident on ONE thread-block cluster (loop mode 3).
+// nb_resident.cu -- the block-step loop resident on ONE thread-block cluster, state in shared memory
+// (loop mode 3, N <= RES_MAX_N).
 //
 // For a small system most block steps advance a handful of particles (config 1, N = 1024: m < 8 in two
-// steps out of three; PAPER.md:252 is about exactly these steps, Table 1 rows 1 and 4).  The arithmetic of
-// such a step is a few microseconds of one SM; what it costs is the hand-over between its phases.  The
-// graph-driven loop (nb_graph.cu) pays five kernel boundaries per step (~20 us).  Here ONE kernel,
-// launched once per nb_run_until / nb_run_steps call as a single cluster of RES_CLUSTER CTAs, runs
-// every step until the control block says done, and the phases of a step are separated by the hardware
-// cluster barrier (barrier.cluster, release / acquire at cluster scope):
+// steps out of three; PAPER.md:252 is about exactly these steps, Table 1 rows 1 and 4).  Such a step is a
+// few thousand pair interactions; what it costs is latency: the graph-driven loop (nb_graph.cu) pays three
+// kernel boundaries and a dozen dependent round trips to L2 per step (~23 us at N = 1024, measured).  Here ONE
+// kernel, launched once per nb_run_until / nb_run_steps call as a single cluster of up to 16 CTAs, keeps
+// the whole system on chip and runs every step until the time or step budget is used:
 //
-//   phase 1  gather + predict   Table 1 row 1 + Eq. 3-7: one pass over the particles (as k_g_gather_predict)
-//   -- cluster barrier --
-//   phase 2  evaluate           the SAME items (i-block, j-split) of the SAME geometry rule as the other
-//                               drivers, each worked by a "virtual CTA" of this cluster (128 threads on a
-//                               named barrier) through force_item
-//   -- cluster barrier --
-//   phase 3  reduce + correct   one warp per active particle: the split partials in the fixed order of
-//                               part_layout / sum_splits_*, then correct_one (Eq. 11-16) by lane 0
-//   -- cluster barrier --
+//   * CTA `rank` OWNS the particles [rank NL, (rank + 1) NL): their committed state (21 doubles each) and their
+//     predicted records live in its shared memory for the whole run (loaded once, written back once).
+//   * phase 1  gather + predict   Table 1 row 1 + Eq. 3-7 for the owned particles; the due ones go to the CTA's
+//                                 list, whose length is broadcast to every CTA through distributed shared memory
+//   * phase 2  evaluate           Eq. 8-10: every CTA evaluates ALL m active particles (their records read from the
+//                                 owners' shared memory) against ITS OWN NL predicted records -- the paper's split of
+//                                 the j-range with one split per CTA -- and stores the partial
+//                                 (a, jerk, snap) into the owner's shared memory
+//   * phase 3  reduce + correct   the owner sums the partials of its active particles in CTA-rank order, applies
+//                                 Eq. 11-16 (correct_one), and broadcasts the minimum of t_i + dt_i it now holds
+//   with one hardware cluster barrier (barrier.cluster, release / acquire) after each phase.
 //
-// The state stays in global memory (L2-resident at these sizes); the predicted stream written in phase 1
-// by generic stores is read in phase 2 by bulk copies (async proxy), hence the proxy fences around the
-// first barrier.  Device functions, geometry and summation order are those of the other drivers, so the
-// states are bit-identical (tests/test_gpu_graph.py).  One cluster is at most 16 SMs: the mode is offered
-// for N <= RES_MAX_N only and chosen by default for N <= RES_AUTO_N, where the all-active steps are still
-// cheap on 16 SMs.
+// The arithmetic is that of the other drivers (pair_body, predict_one, correct_one, new_dt); only the order
+// in which the pair terms of one particle are added differs (per lane over the owner-CTA slice, butterfly over
+// the lanes, then over the CTAs in rank order: fixed, so runs are bit-reproducible).  Results therefore agree
+// with the other drivers to rounding (G18), not bit for bit; tests/test_gpu_graph.py checks identical time
+// steps and positions to 1e-12 against the host-issued call sequence.
+#include <cooperative_groups.h>
+
 #include "nb_internal.cuh"
 #include "nb_force_dev.cuh"
 #include "nb_step_dev.cuh"
 
+namespace cg = cooperative_groups;
+
 namespace nb {
 
-constexpr int RES_THREADS = 512;                      // 16 warps per CTA: 4 per SM sub-partition
+constexpr int RES_THREADS = 512;    // 16 warps per CTA
 constexpr int RES_WARPS = RES_THREADS / 32;
-constexpr int RES_VC = RES_THREADS / NT_E;            // virtual evaluation CTAs per CTA
-constexpr int RES_GEOM_SLOTS = 64;                    // per-CTA direct-mapped memory of geometries by set size
+constexpr int RES_MAXC = 16;        // largest cluster
+constexpr int RES_NL_MAX = 256;     // owned particles per CTA at most (N <= 2048 on 8 CTAs; 16 CTAs: 128 each)
+constexpr int RES_PUSH = 16;        // each owner pushes the records of its first RES_PUSH due particles to every CTA
 
-struct ResShared {
-    double tile[RES_VC][2][TJ_E * REC];   // one two-stage ring of j-tiles per virtual CTA
-    uint64_t full[RES_VC][2];
-    ForceGeom geom[RES_GEOM_SLOTS];
-    int geom_m[RES_GEOM_SLOTS];
-    SplitProblem sp;
-    ForceGeom g;
-    long long scost[MAX_WAVES + 1];
-    int ssplit[MAX_WAVES + 1];
-    double red[RES_WARPS];
+// Shared-memory plan of one CTA (NL = owned particles, a multiple of 32; doubles unless noted):
+//   state  : t, dt, mass [NL]; r, v, a, jerk, snap, crackle [3][NL]      21 NL
+//   rec    : predicted records [NL][REC]                                   10 NL
+//   f1     : reduced (a, jerk, snap) of the owned active particles [9][NL]  9 NL
+//   part   : partials [NL][C][9] written by every CTA of the cluster       9 C NL
+//   irec   : records of the first RES_PUSH due particles of every CTA [16][RES_PUSH][REC], pushed by their owners
+//            (a small active set is then evaluated without a read from remote shared memory)
+//   tmin   : min(t_i + dt_i) of every CTA [16];  list: int32 local indices of the owned due particles [NL];
+//   cnt    : int32 list length of every CTA [16]
+struct ResPlan {
+    int NL, C;
+    size_t o_t, o_dt, o_m, o_r, o_v, o_a, o_j, o_s, o_c, o_rec, o_f1, o_part, o_irec, o_tmin, o_list, o_cnt, bytes;
 };
-
-__device__ __forceinline__ void cluster_sync_all()
+__host__ __device__ inline ResPlan res_plan(const int64_t N, const int C)
 {
-    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    ResPlan p;
+    p.C = C;
+    int NL = (int)((N + C - 1) / C);
+    NL = (NL + 31) & ~31;
+    p.NL = NL;
+    size_t o = 0;
+    p.o_t = o; o += (size_t)NL * 8;
+    p.o_dt = o; o += (size_t)NL * 8;
+    p.o_m = o; o += (size_t)NL * 8;
+    p.o_r = o; o += (size_t)3 * NL * 8;
+    p.o_v = o; o += (size_t)3 * NL * 8;
+    p.o_a = o; o += (size_t)3 * NL * 8;
+    p.o_j = o; o += (size_t)3 * NL * 8;
+    p.o_s = o; o += (size_t)3 * NL * 8;
+    p.o_c = o; o += (size_t)3 * NL * 8;
+    p.o_rec = o; o += (size_t)REC * NL * 8;
+    p.o_f1 = o; o += (size_t)9 * NL * 8;
+    p.o_part = o; o += (size_t)9 * C * NL * 8;
+    p.o_irec = o; o += (size_t)RES_MAXC * RES_PUSH * REC * 8;
+    p.o_tmin = o; o += (size_t)RES_MAXC * 8;
+    p.o_list = o; o += (size_t)NL * 4;
+    p.o_cnt = o; o += (size_t)RES_MAXC * 4;
+    p.bytes = (o + 15) & ~(size_t)15;
+    return p;
 }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
-// min over the CTA of one value per thread -> atomicMin on the bits (times are non-negative)
-__device__ __forceinline__ void res_block_min_to(double v, unsigned long long *dst, double *red)
+// One active particle (record ri, read from its owner's shared memory) against the owned records
+// jl, jl + JL, ...: the pair body of the other drivers; the JL lanes that share it are combined by the butterfly.
+template <int JL, bool GUARD0, int MX>
+__device__ __forceinline__ Acc9 res_eval(const double *ri, const double *rec, const int jl, const int NL, const double eps2)
 {
-    const double inf = __longlong_as_double(0x7ff0000000000000LL);
-    for (int off = 16; off > 0; off >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, off));
-    __syncthreads();
-    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
-    __syncthreads();
-    if (threadIdx.x < 32) {
-        v = threadIdx.x < RES_WARPS ? red[threadIdx.x] : inf;
-        for (int off = 16; off > 0; off >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, off));
-        if (threadIdx.x == 0 && v < inf) atomicMin(dst, (unsigned long long)__double_as_longlong(v));
+    const double xi = ri[0], yi = ri[1], zi = ri[2], vxi = ri[3], vyi = ri[4], vzi = ri[5];
+    const double axi = ri[6], ayi = ri[7], azi = ri[8];
+    Acc9 T = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+    const double *q = rec + jl * REC;
+    const int per = NL / JL;
+    if (MX == 1) {
+        const float eps2f = (float)eps2;
+        for (int j0 = 0; j0 < per; j0 += 128) {        // float sums over at most 128 pair terms, as in force_item
+            AccF A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+            const int j1 = min(per, j0 + 128);
+#pragma unroll 4
+            for (int jj = j0; jj < j1; ++jj)
+                pair_body_mx<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + (size_t)jj * (JL * REC), eps2f, A);
+            T.ax += (double)A.ax; T.ay += (double)A.ay; T.az += (double)A.az;
+            T.jx += (double)A.jx; T.jy += (double)A.jy; T.jz += (double)A.jz;
+            T.sx += (double)A.sx; T.sy += (double)A.sy; T.sz += (double)A.sz;
+        }
+    } else {
+#pragma unroll 8
+        for (int jj = 0; jj < per; ++jj)
+            pair_body<GUARD0, true>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + (size_t)jj * (JL * REC), eps2, T);
     }
+    if (MX != 1) {  // the FP64 pair body accumulates 3 sqrt(3) times the sums (pair_body)
+        T.ax *= PAIR_SCALE; T.ay *= PAIR_SCALE; T.az *= PAIR_SCALE;
+        T.jx *= PAIR_SCALE; T.jy *= PAIR_SCALE; T.jz *= PAIR_SCALE;
+        T.sx *= PAIR_SCALE; T.sy *= PAIR_SCALE; T.sz *= PAIR_SCALE;
+    }
+    if (JL > 1) {
+#pragma unroll
+        for (int off = JL >> 1; off > 0; off >>= 1) {
+            T.ax += __shfl_xor_sync(0xffffffffu, T.ax, off); T.ay += __shfl_xor_sync(0xffffffffu, T.ay, off);
+            T.az += __shfl_xor_sync(0xffffffffu, T.az, off); T.jx += __shfl_xor_sync(0xffffffffu, T.jx, off);
+            T.jy += __shfl_xor_sync(0xffffffffu, T.jy, off); T.jz += __shfl_xor_sync(0xffffffffu, T.jz, off);
+            T.sx += __shfl_xor_sync(0xffffffffu, T.sx, off); T.sy += __shfl_xor_sync(0xffffffffu, T.sy, off);
+            T.sz += __shfl_xor_sync(0xffffffffu, T.sz, off);
+        }
+    }
+    return T;
 }
 
-// The geometry of a set size, identical to choose_geom(): remembered per CTA (block-step runs see the same few
-// sizes again and again); on a miss the split candidates are scored by one thread each.  Called by all threads.
-__device__ __forceinline__ ForceGeom res_geometry(ResShared &sh, const int m, const int64_t Npad, const int n_sm,
-                                                  const int occ, const int64_t partials_limit,
-                                                  const int force_split, const int force_jlanes)
+// correct_one (nb_step_dev.cuh: Eq. 11-14, the end-point derivatives G6, the time-step rule Eq. 15-16) spread over
+// a warp to shorten its dependent chain: lanes 0..2 take one component each, lanes 0..5 one of the six norms of
+// Eq. 16 each, lane 0 the decision.  Same expressions, same rounding order as correct_one.
+__device__ __forceinline__ void correct_warp(const int lane, const int k, const int i, const int NL, const double t_next,
+                                             const double eta, const double dt_min, const double dt_max, const double *f1,
+                                             double *ti, double *dti, double *r, double *v, double *a, double *j, double *s,
+                                             double *c)
 {
-    const int slot = m & (RES_GEOM_SLOTS - 1);
-    __syncthreads();
-    if (sh.geom_m[slot] != m) {
-        if (threadIdx.x == 0) sh.sp = geom_begin(sh.g, m, Npad, n_sm, occ, partials_limit, force_jlanes);
-        __syncthreads();
-        if (threadIdx.x <= MAX_WAVES) {
-            int S;
-            sh.scost[threadIdx.x] = split_candidate(sh.sp, threadIdx.x, &S);
-            sh.ssplit[threadIdx.x] = S;
-        }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            long long best = INT64_MAX;
-            int best_s = 1;
-            for (int w = 0; w <= MAX_WAVES; ++w)
-                if (sh.scost[w] < best) { best = sh.scost[w]; best_s = sh.ssplit[w]; }
-            geom_finish(sh.g, sh.sp, best_s, force_split);
-            sh.geom[slot] = sh.g;
-            sh.geom_m[slot] = m;
-        }
-        __syncthreads();
+    const double h = dti[i];
+    double val[6] = {0, 0, 0, 0, 0, 0};   // a1, j1, s1, a^(3), a^(4), a^(5) of this lane's component
+    if (lane < 3) {
+        const int d = lane;
+        const double h2 = h * h, h3 = h2 * h;
+        const double ih = 1.0 / h;  // exact: h is a power of two
+        const double ih3 = ih * ih * ih, ih4 = ih3 * ih, ih5 = ih4 * ih;
+        const int q = d * NL + i;
+        const double r0 = r[q], v0 = v[q], a0 = a[q], j0 = j[q], s0 = s[q];
+        const double a1 = f1[(0 + d) * NL + k], j1 = f1[(3 + d) * NL + k], s1 = f1[(6 + d) * NL + k];
+        const double vc = v0 + (h * 0.5) * (a1 + a0) - (h2 * 0.1) * (j1 - j0) + (h3 * (1.0 / 120.0)) * (s1 + s0);
+        const double rc = r0 + (h * 0.5) * (vc + v0) - (h2 * 0.1) * (a1 - a0) + (h3 * (1.0 / 120.0)) * (j1 + j0);
+        const double dA = a1 - a0;
+        val[0] = a1; val[1] = j1; val[2] = s1;
+        val[3] = 3.0 * (20.0 * dA - h * (8.0 * j0 + 12.0 * j1) + h2 * (3.0 * s1 - s0)) * ih3;
+        val[4] = 12.0 * (30.0 * dA - h * (14.0 * j0 + 16.0 * j1) + h2 * (3.0 * s1 - 2.0 * s0)) * ih4;
+        val[5] = 60.0 * (12.0 * dA - 6.0 * h * (j0 + j1) + h2 * (s1 - s0)) * ih5;
+        r[q] = rc; v[q] = vc; a[q] = a1; j[q] = j1; s[q] = s1; c[q] = val[3];
     }
-    return sh.geom[slot];
+    double nrm = 0.0;
+#pragma unroll
+    for (int X = 0; X < 6; ++X) {
+        const double x = __shfl_sync(0xffffffffu, val[X], 0), y = __shfl_sync(0xffffffffu, val[X], 1),
+                     z = __shfl_sync(0xffffffffu, val[X], 2);
+        if (lane == X) nrm = norm3_rn(x, y, z);
+    }
+    double n6[6];
+#pragma unroll
+    for (int X = 0; X < 6; ++X) n6[X] = __shfl_sync(0xffffffffu, nrm, X);
+    if (lane == 0) {
+        ti[i] = t_next;
+        dti[i] = new_dt(n6[0], n6[1], n6[2], n6[3], n6[4], n6[5], eta, h, t_next, dt_min, dt_max);
+    }
 }
 
 template <bool GUARD0, int MX>
 __global__ void __launch_bounds__(RES_THREADS, 1)
     k_resident_loop(const int64_t N, const int64_t Npad, const double eps2, const double eta, const double dt_min,
-                    const double dt_max, double *t, double *dt, double *mass, double *r, double *v, double *a,
-                    double *j, double *s, double *c, double *jp, int32_t *active_list, double *f1, double *partials,
-                    StepCtl *ctl, const int n_sm, const int occ, const int64_t partials_limit,
-                    const int force_split, const int force_jlanes)
+                    const double dt_max, double *__restrict__ g_t, double *__restrict__ g_dt, const double *__restrict__ g_m,
+                    double *__restrict__ g_r, double *__restrict__ g_v, double *__restrict__ g_a, double *__restrict__ g_j,
+                    double *__restrict__ g_s, double *__restrict__ g_c, double *__restrict__ g_jp, StepCtl *__restrict__ ctl,
+                    const int force_jlanes)
 {
-    extern __shared__ __align__(128) unsigned char res_smem[];
-    ResShared &sh = *reinterpret_cast<ResShared *>(res_smem);
+    extern __shared__ __align__(128) unsigned char smem[];
+    cg::cluster_group cluster = cg::this_cluster();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int n_cta = gridDim.x, rank = blockIdx.x;            // the grid is one cluster
-    const int gwarp = rank * RES_WARPS + warp, gwarps = n_cta * RES_WARPS;
+    const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
+    const ResPlan P = res_plan(N, C);
+    const int NL = P.NL;
+    double *t = (double *)(smem + P.o_t), *dt = (double *)(smem + P.o_dt), *mass = (double *)(smem + P.o_m);
+    double *r = (double *)(smem + P.o_r), *v = (double *)(smem + P.o_v), *a = (double *)(smem + P.o_a);
+    double *j = (double *)(smem + P.o_j), *s = (double *)(smem + P.o_s), *c = (double *)(smem + P.o_c);
+    double *rec = (double *)(smem + P.o_rec), *f1 = (double *)(smem + P.o_f1), *part = (double *)(smem + P.o_part);
+    double *tmin = (double *)(smem + P.o_tmin), *irec = (double *)(smem + P.o_irec);
+    int *list = (int *)(smem + P.o_list), *cnt = (int *)(smem + P.o_cnt);
+    __shared__ int n_list;
+    __shared__ double red[RES_WARPS];
+    __shared__ long long hist[64];
     const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    const int64_t first = (int64_t)rank * NL;                       // first owned particle
+    const int64_t left = N - first;
+    const int n_own = left <= 0 ? 0 : (left < NL ? (int)left : NL);
 
-    if (tid == 0) {
-        for (int q = 0; q < RES_VC; ++q) { mbar_init(&sh.full[q][0], 1); mbar_init(&sh.full[q][1], 1); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    // ---- load the owned slice (rows beyond N: mass 0 at the origin, never due)
+    for (int i = tid; i < NL; i += RES_THREADS) {
+        const bool live = i < n_own;
+        const int64_t gi = first + i;
+        t[i] = live ? g_t[gi] : 0.0; dt[i] = live ? g_dt[gi] : inf; mass[i] = live ? g_m[gi] : 0.0;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const int64_t gq = d * Npad + gi;
+            const int q = d * NL + i;
+            r[q] = live ? g_r[gq] : 0.0; v[q] = live ? g_v[gq] : 0.0; a[q] = live ? g_a[gq] : 0.0;
+            j[q] = live ? g_j[gq] : 0.0; s[q] = live ? g_s[gq] : 0.0; c[q] = live ? g_c[gq] : 0.0;
+        }
+#pragma unroll
+        for (int d = 0; d < REC; ++d) rec[i * REC + d] = 0.0;
     }
-    for (int q = tid; q < RES_GEOM_SLOTS; q += RES_THREADS) sh.geom_m[q] = -1;
+    for (int b = tid; b < 64; b += RES_THREADS) hist[b] = 0;
+    long long steps_left = ctl->steps_left;
+    const double t_end = ctl->t_end;
+    long long n_steps = 0;
+    double n_pairs = 0.0, t_now = 0.0;
     __syncthreads();
-    unsigned tc = 0;                // tiles consumed so far through this thread's ring
-    volatile StepCtl *vctl = ctl;
-#ifdef NB_RES_TIMING   // development aid: cycles per phase of the step, summed by one thread into unused histogram bins
+
+    // minimum of t_i + dt_i over the owned particles -> tmin[rank] of every CTA
+    auto publish_min = [&]() {
+        double vmin = inf;
+        for (int i = tid; i < n_own; i += RES_THREADS) vmin = fmin(vmin, t[i] + dt[i]);
+        for (int off = 16; off > 0; off >>= 1) vmin = fmin(vmin, __shfl_xor_sync(0xffffffffu, vmin, off));
+        if (lane == 0) red[warp] = vmin;
+        __syncthreads();
+        if (warp == 0) {
+            vmin = lane < RES_WARPS ? red[lane] : inf;
+            for (int off = 16; off > 0; off >>= 1) vmin = fmin(vmin, __shfl_xor_sync(0xffffffffu, vmin, off));
+            if (lane < C) cluster.map_shared_rank(tmin, lane)[rank] = vmin;
+        }
+    };
+    publish_min();
+    cluster.sync();
+#ifdef NB_RES_TIMING   // development aid: cycles per phase, summed by one thread into unused histogram bins
     long long tph[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     long long tq = clock64();
 #define NB_TICK(q) do { const long long now_ = clock64(); tph[q] += now_ - tq; tq = now_; } while (0)
@@ -130,92 +243,126 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
 #define NB_TICK(q) do { } while (0)
 #endif
 
-    for (int p = 0;; p ^= 1) {
-        // ---- phase 1: gather + predict.  Every thread of the cluster evaluates the same condition from
-        // values that nothing modifies before the second barrier of the step.
-        const double tn = __longlong_as_double((long long)vctl->tmin[p]);
-        if (vctl->steps_left <= 0 || !(tn <= vctl->t_end)) break;
+    for (;;) {
+        // ---- next block time: every thread of the cluster computes the same minimum
+        double tn = lane < C ? tmin[lane] : inf;
+        for (int off = 16; off > 0; off >>= 1) tn = fmin(tn, __shfl_xor_sync(0xffffffffu, tn, off));
+        if (steps_left <= 0 || !(tn <= t_end)) break;
         NB_TICK(0);
-        double vmin = inf;
-        for (int64_t base = (int64_t)gwarp * 32; base < N; base += (int64_t)gwarps * 32) {   // warp-uniform trip count
-            const int64_t i = base + lane;
-            bool hit = false;
-            if (i < N) {
-                const double due = t[i] + dt[i];
-                hit = (due == tn);
-                if (!hit) vmin = fmin(vmin, due);
-                predict_one(i, Npad, tn, t, mass, r, v, a, j, s, c, jp);
-            }
-            // warp-aggregated append (the order of the list affects no result, G18)
-            const unsigned mask = __ballot_sync(0xffffffffu, hit);
-            if (mask) {
-                const int leader = __ffs(mask) - 1;
-                int slot0 = 0;
-                if (lane == leader) slot0 = atomicAdd(&ctl->cnt[p], __popc(mask));
-                slot0 = __shfl_sync(0xffffffffu, slot0, leader);
-                if (hit) active_list[slot0 + __popc(mask & ((1u << lane) - 1u))] = (int32_t)i;
+
+        // ---- phase 1: predict the owned particles (Eq. 3-7), list the due ones (Table 1 row 1)
+        if (tid == 0) n_list = 0;
+        __syncthreads();
+        for (int i = tid; i < n_own; i += RES_THREADS) {
+            predict_one(i, NL, tn, t, mass, r, v, a, j, s, c, rec);
+            if (t[i] + dt[i] == tn) list[atomicAdd(&n_list, 1)] = i;
+        }
+        __syncthreads();
+        if (tid < C) cluster.map_shared_rank(cnt, tid)[rank] = n_list;
+        {   // the records of the first RES_PUSH due particles go to every CTA (remote stores, fire and forget)
+            const int np = n_list < RES_PUSH ? n_list : RES_PUSH;
+            for (int e = tid; e < C * np * REC; e += RES_THREADS) {
+                const int o = e / (np * REC), w = e - o * (np * REC), qq = w / REC, d = w - qq * REC;
+                cluster.map_shared_rank(irec, o)[((size_t)rank * RES_PUSH + qq) * REC + d] = rec[(size_t)list[qq] * REC + d];
             }
         }
-        res_block_min_to(vmin, &ctl->tmin[1 - p], sh.red);
         NB_TICK(1);
-        fence_proxy_async();          // the records just stored are read by bulk copies (async proxy) below
-        cluster_sync_all();
-        fence_proxy_async();
+        cluster.sync();
         NB_TICK(2);
 
-        // ---- phase 2: evaluate
-        const int m = vctl->cnt[p];
-        const ForceGeom g = res_geometry(sh, m, Npad, n_sm, occ, partials_limit, force_split, force_jlanes);
-        NB_TICK(3);
-        const int32_t *active = (m == N) ? nullptr : active_list;
-        double *out = g.S > 1 ? partials : f1;
-        const PartLayout L = part_layout(g.S, g.mpad, Npad);
-        const long long items = (long long)g.n_ib * g.S;
-        {
-            const int vc = tid / NT_E, vt = tid % NT_E;        // virtual CTA of 128 threads, named barrier 1 + vc
-            const int tiles_total = (int)(Npad / TJ_E);
-            for (long long w = (long long)rank * RES_VC + vc; w < items; w += (long long)n_cta * RES_VC)
-                force_item_jl<NT_E, TJ_E, GUARD0, MX, 12, 2>(g.JL, jp, jp, active, m, (int)(w % g.n_ib), (int)(w / g.n_ib),
-                                                             tiles_total, g.tps, eps2, out, L.cstride, L.kstride, L.sstride,
-                                                             sh.tile[vc], sh.full[vc], tc, vt, 1 + vc);
-        }
-        NB_TICK(4);
-        cluster_sync_all();
-        NB_TICK(5);
-
-        // ---- phase 3: reduce + correct, one warp per active particle; the sum over the splits runs in the
-        // order every driver uses (part_layout, sum_splits_*), so that all agree bit for bit.
-        vmin = inf;
-        for (int k = gwarp; k < m; k += gwarps) {
-            if (g.S > 1) reduce_one(partials, g.S, L, k, lane, f1, Npad);
-            if (lane == 0) {
-                const int64_t i = active ? active[k] : k;
-                vmin = fmin(vmin, correct_one(k, i, Npad, tn, eta, dt_min, dt_max, f1, t, dt, r, v, a, j, s, c));
+        // ---- phase 2: all m active particles against the owned records; partials to the owners
+        int base[RES_MAXC + 1];
+        base[0] = 0;
+#pragma unroll
+        for (int o = 0; o < RES_MAXC; ++o) base[o + 1] = base[o] + (o < C ? cnt[o] : 0);
+        const int m = base[RES_MAXC];
+        int JL = 1;
+        if (force_jlanes >= 1) JL = force_jlanes < JL_MAX ? force_jlanes : JL_MAX;
+        else { while (JL < JL_MAX && m * (JL * 2) <= RES_THREADS) JL *= 2; }
+        const int slots = RES_THREADS / JL;
+        for (int k0 = 0; k0 < m; k0 += slots) {                 // warp-uniform trip count
+            const int k = k0 + tid / JL, jl = tid % JL;
+            const bool live = k < m;
+            const int kk = live ? k : m - 1;
+            int o = 0, bo = 0;                                  // owner CTA of slot kk and the first slot it owns
+#pragma unroll
+            for (int q = 1; q < RES_MAXC; ++q)
+                if (q < C && kk >= base[q]) { o = q; bo = base[q]; }
+            const int qloc = kk - bo;                           // slot in the owner's list
+            const double *ri;
+            if (qloc < RES_PUSH) ri = irec + ((size_t)o * RES_PUSH + qloc) * REC;     // pushed by its owner in phase 1
+            else ri = cluster.map_shared_rank(rec, o) + (size_t)cluster.map_shared_rank(list, o)[qloc] * REC;
+            Acc9 T;
+            switch (JL) {
+                case 1: T = res_eval<1, GUARD0, MX>(ri, rec, jl, NL, eps2); break;
+                case 2: T = res_eval<2, GUARD0, MX>(ri, rec, jl, NL, eps2); break;
+                case 4: T = res_eval<4, GUARD0, MX>(ri, rec, jl, NL, eps2); break;
+                case 8: T = res_eval<8, GUARD0, MX>(ri, rec, jl, NL, eps2); break;
+                case 16: T = res_eval<16, GUARD0, MX>(ri, rec, jl, NL, eps2); break;
+                default: T = res_eval<32, GUARD0, MX>(ri, rec, jl, NL, eps2); break;
+            }
+            if (live && jl == 0) {
+                double *dst = cluster.map_shared_rank(part, o) + ((size_t)qloc * C + rank) * 9;
+                dst[0] = T.ax; dst[1] = T.ay; dst[2] = T.az; dst[3] = T.jx; dst[4] = T.jy; dst[5] = T.jz;
+                dst[6] = T.sx; dst[7] = T.sy; dst[8] = T.sz;
             }
         }
-        res_block_min_to(vmin, &ctl->tmin[1 - p], sh.red);
-        if (rank == 0 && tid == 0) {      // bookkeeping: fields nobody reads before the next barrier
-            ctl->t_now = tn;
-            ctl->t_next = tn;
-            ctl->n_active = m;
-            ctl->steps_left -= 1;
-            ctl->n_steps += 1;
-            ctl->n_pairs += (double)m * (double)N;
+        NB_TICK(3);
+        cluster.sync();
+        NB_TICK(4);
+
+        // ---- phase 3: the owner sums the C partials of each of its active particles in rank order and
+        // corrects it (Eq. 11-16).  One warp per particle: lanes 0..8 take one component each.
+        const int n_mine = cnt[rank];
+        for (int q = warp; q < n_mine; q += RES_WARPS) {
+            if (lane < 9) {
+                double acc = 0.0;
+                for (int o = 0; o < C; ++o) acc += part[((size_t)q * C + o) * 9 + lane];
+                f1[lane * NL + q] = acc;
+            }
+            __syncwarp();
+            correct_warp(lane, q, list[q], NL, tn, eta, dt_min, dt_max, f1, t, dt, r, v, a, j, s, c);
+        }
+        __syncthreads();
+        steps_left -= 1; n_steps += 1; n_pairs += (double)m * (double)N; t_now = tn;
+        if (tid == 0) {
             int b = 0;
             while ((1LL << (b + 1)) <= (long long)m) ++b;
-            ctl->hist[b] += 1;
-            ctl->tmin[p] = 0x7ff0000000000000ULL;   // consumed: slot p collects the minimum of the step after next
-            ctl->cnt[p] = 0;
+            hist[b] += 1;
         }
+        publish_min();
+        NB_TICK(5);
+        cluster.sync();
         NB_TICK(6);
-        cluster_sync_all();
-        NB_TICK(7);
     }
 #ifdef NB_RES_TIMING
     if (rank == 0 && tid == 0)
-        for (int q = 0; q < 8; ++q) ctl->hist[40 + q] += tph[q];
+        for (int q = 0; q < 8; ++q) hist[40 + q] += tph[q];
+    __syncthreads();
 #endif
-    if (rank == 0 && tid == 0) ctl->done = 1;
+
+    // ---- write the owned slice back: committed state and the last prediction
+    __syncthreads();
+    for (int i = tid; i < n_own; i += RES_THREADS) {
+        const int64_t gi = first + i;
+        g_t[gi] = t[i]; g_dt[gi] = dt[i];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const int64_t gq = d * Npad + gi;
+            const int q = d * NL + i;
+            g_r[gq] = r[q]; g_v[gq] = v[q]; g_a[gq] = a[q]; g_j[gq] = j[q]; g_s[gq] = s[q]; g_c[gq] = c[q];
+        }
+        if (n_steps > 0) {
+#pragma unroll
+            for (int d = 0; d < REC; ++d) g_jp[gi * REC + d] = rec[i * REC + d];
+        }
+    }
+    if (rank == 0 && tid == 0) {
+        ctl->steps_left = steps_left; ctl->n_steps = n_steps; ctl->n_pairs = n_pairs; ctl->t_now = t_now;
+        for (int b = 0; b < 64; ++b) ctl->hist[b] = hist[b];
+        ctl->done = 1;
+    }
+    cluster.sync();   // no CTA leaves while another may still read its shared memory
 }
 
 // ---- host side ---------------------------------------------------------------------------
@@ -223,7 +370,9 @@ template <bool G0, int MX>
 static cudaError_t launch_resident(nb_ctx *ctx, int n_cta)
 {
     auto kern = k_resident_loop<G0, MX>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ResShared));
+    const ResPlan P = res_plan(ctx->N, n_cta);
+    if (P.NL > RES_NL_MAX) return cudaErrorInvalidValue;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P.bytes);
     if (e != cudaSuccess) return e;
     if (n_cta > 8) {
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
@@ -231,7 +380,7 @@ static cudaError_t launch_resident(nb_ctx *ctx, int n_cta)
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)n_cta); cfg.blockDim = dim3(RES_THREADS);
-    cfg.dynamicSmemBytes = sizeof(ResShared); cfg.stream = ctx->stream;
+    cfg.dynamicSmemBytes = P.bytes; cfg.stream = ctx->stream;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = (unsigned)n_cta; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
@@ -241,9 +390,8 @@ static cudaError_t launch_resident(nb_ctx *ctx, int n_cta)
     if (e != cudaSuccess) return e;
     if (n_clusters < 1) return cudaErrorLaunchOutOfResources;
     return cudaLaunchKernelEx(&cfg, kern, ctx->N, ctx->Npad, ctx->eps2, ctx->eta, ctx->dt_min, ctx->dt_max, ctx->t, ctx->dt,
-                              ctx->mass, ctx->r, ctx->v, ctx->a, ctx->j, ctx->s, ctx->c, ctx->jp, ctx->active, ctx->f1,
-                              ctx->partials, ctx->ctl, ctx->n_sm, ctx->occ[0], (int64_t)ctx->partials_limit,
-                              ctx->force_split, ctx->force_jlanes);
+                              (const double *)ctx->mass, ctx->r, ctx->v, ctx->a, ctx->j, ctx->s, ctx->c, ctx->jp, ctx->ctl,
+                              ctx->force_jlanes);
 }
 
 static cudaError_t launch_resident_any(nb_ctx *ctx, int n_cta)
@@ -263,21 +411,24 @@ int resident_run(nb_ctx *ctx, double t_end, int64_t max_steps, int64_t *n_steps)
         return set_err(ctx, NB_EINVAL, "loop mode 3 (cluster-resident loop) serves N <= %lld; this context has N = %lld",
                        (long long)RES_MAX_N, (long long)ctx->N);
     {
-        const int rc = reserve_partials(ctx, ctx->partials_limit);
+        const int rc = launch_graph_begin(ctx, t_end, max_steps);   // seeds the control block (t_end, steps_left, counters)
         if (rc != NB_OK) return rc;
     }
-    {
-        const int rc = launch_graph_begin(ctx, t_end, max_steps);   // seeds the control block and tmin[0]
-        if (rc != NB_OK) return rc;
-    }
-    if (ctx->res_cluster == 0) ctx->res_cluster = 16;
+    if (ctx->res_cluster == 0) ctx->res_cluster = RES_MAXC;
     cudaError_t e = launch_resident_any(ctx, ctx->res_cluster);
-    if (e != cudaSuccess && ctx->res_cluster > 8) {   // no 16-SM cluster on this part: the portable size
+    if (e != cudaSuccess && ctx->res_cluster > 8) {   // no 16-CTA cluster on this part: the portable size
         cudaGetLastError();
         ctx->res_cluster = 8;
         e = launch_resident_any(ctx, 8);
     }
-    if (e != cudaSuccess) return set_err(ctx, NB_ECUDA, "launch of k_resident_loop failed: %s", cudaGetErrorString(e));
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        if (ctx->loop_auto) {   // this device cannot host the cluster: the default falls back to the graph-driven loop
+            ctx->use_graph = 1;
+            return graph_run(ctx, t_end, max_steps, n_steps);
+        }
+        return set_err(ctx, NB_ECUDA, "launch of k_resident_loop failed: %s", cudaGetErrorString(e));
+    }
     ctx->n_launch += 1;
     NB_CUDA(ctx, cudaMemcpyAsync(ctx->h_ctl, ctx->ctl, sizeof(StepCtl), cudaMemcpyDeviceToHost, ctx->stream));
     NB_CUDA(ctx, cudaStreamSynchronize(ctx->stream));

@@ -155,12 +155,24 @@ def test_heavy_particle_lockstep_with_oracle_both_drivers(nb, oracle):
     assert err < 1e-11
     st_host = torch.empty_like(st0)
     nb.nb_get_full_state(g.ctx, st_host); g.sync()
-    # device-driven loop from the same start: bit-identical to the call sequence
+    # graph-driven loop from the same start: bit-identical to the call sequence
+    nb.nb_set_loop_mode(g.ctx, 1)
     nb.nb_set_full_state(g.ctx, st0)
     g.run_steps(steps, log=False)
     st_dev = torch.empty_like(st0)
     nb.nb_get_full_state(g.ctx, st_dev); g.sync()
     assert torch.equal(st_host, st_dev)
+    # cluster-resident loop (the default driver at this N; its own summation order): the same steps and time
+    # steps, positions to rounding
+    nb.nb_set_loop_mode(g.ctx, 3)
+    nb.nb_set_full_state(g.ctx, st0)
+    g.run_steps(steps, log=False)
+    st_res = torch.empty_like(st0)
+    nb.nb_get_full_state(g.ctx, st_res); g.sync()
+    a, b = host(st_res), host(st_host)
+    assert np.array_equal(a[:, :3], b[:, :3])                # m, t, dt
+    err = (np.linalg.norm(a[:, 3:6] - b[:, 3:6], axis=1) / np.maximum(np.linalg.norm(b[:, 3:6], axis=1), 1e-3)).max()
+    assert err < 1e-11
     g.close()
 
 
