@@ -194,9 +194,11 @@ int nb_set_forces(nb_ctx *ctx, const double *buf);
 /* Arithmetic of the evaluation step.  0 (default): IEEE binary64 throughout.  1: the paper's own
  * mixed scheme (section 5.7): predicted data stay double, the nine differences
  * r_ij, v_ij, a_ij are formed in double and rounded to float, the pair arithmetic of Eq. 8-10 is
- * float, pair terms are summed in float within a j-tile (64 or 128 j) and the tile sums in double
- * (reading G27).  Relative error of a force ~1e-7 of sum_j |pair term| instead of
- * ~1e-16; everything else (predictor, corrector, time steps, energy) stays binary64.        */
+ * float, pair terms are summed in float within a j-tile (at most 128 j) and the tile sums in double
+ * (reading G27).  2: the same, but the acceleration and jerk terms of every pair are added in
+ * double -- 9 + 6 = the 15 double-precision operations per pair that PAPER.md:301 counts (reading G27b).
+ * Relative error of a force ~1e-7 of sum_j |pair term| instead of ~1e-16; everything else (predictor,
+ * corrector, time steps, energy) stays binary64.                                            */
 int nb_set_precision(nb_ctx *ctx, int mode);
 
 /* Debug switch (Errors): 1 = nb_force range-checks a caller-supplied

@@ -516,7 +516,8 @@ extern "C" int nb_set_forces(nb_ctx *ctx, const double *buf)
 extern "C" int nb_set_precision(nb_ctx *ctx, int mode)
 {
     if (!ctx) return NB_EINVAL;
-    if (mode != 0 && mode != 1) return set_err(ctx, NB_EINVAL, "nb_set_precision: 0 (FP64) or 1 (mixed SP/DP)");
+    if (mode < 0 || mode > 2)
+        return set_err(ctx, NB_EINVAL, "nb_set_precision: 0 (FP64), 1 (mixed SP/DP) or 2 (mixed, acceleration and jerk summed in double)");
     ctx->precision = mode;
     ctx->evaluated = false; ctx->eval_partial = false;
     return NB_OK;

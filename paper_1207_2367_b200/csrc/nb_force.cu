@@ -171,10 +171,12 @@ static void launch_lanes(nb_ctx *ctx, dim3 grid, const int32_t *active, int m, i
 #define NB_KF(G0, MXP)                                                                                              \
     k_force<JL, G0, MXP><<<grid, NT_E, 0, ctx->stream>>>(ctx->jp, jstream, active, m, tiles_total, tps, ctx->eps2, out, \
                                                           L.cstride, L.kstride, L.sstride)
-    const bool mx = ctx->precision == 1;
+    const int mx = ctx->precision == 1 ? 1 : (ctx->precision == 2 ? 3 : 0);   // kernel template value (force_item)
     const bool g0 = mx ? mx_needs_guard(ctx) : ctx->eps == 0.0;
-    if (g0 && mx) NB_KF(true, 1);
-    else if (mx) NB_KF(false, 1);
+    if (g0 && mx == 1) NB_KF(true, 1);
+    else if (mx == 1) NB_KF(false, 1);
+    else if (g0 && mx == 3) NB_KF(true, 3);
+    else if (mx == 3) NB_KF(false, 3);
     else if (JL == 1 && no_snap) {     // start-up pass 1 of a large system; small ones take the full body (same a, jerk)
         if (g0) NB_KF(true, 2);
         else NB_KF(false, 2);
@@ -231,11 +233,14 @@ int enqueue_force_persistent(nb_ctx *ctx)
 #define NB_KP(G0, MXP)                                                                                      \
     launch_chain(k_force_persistent<G0, MXP>, dim3(gP), dim3(NT_E), ctx->stream, pdl, ctx->jp, ctx->active, \
                  ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl)
-    const bool mx = ctx->precision == 1, pdl = ctx->use_graph == 2;
+    const int mx = ctx->precision == 1 ? 1 : (ctx->precision == 2 ? 3 : 0);
+    const bool pdl = ctx->use_graph == 2;
     const bool g0 = mx ? mx_needs_guard(ctx) : ctx->eps == 0.0;
-    if (g0 && mx) NB_KP(true, 1);
+    if (g0 && mx == 1) NB_KP(true, 1);
+    else if (g0 && mx == 3) NB_KP(true, 3);
     else if (g0) NB_KP(true, 0);
-    else if (mx) NB_KP(false, 1);
+    else if (mx == 1) NB_KP(false, 1);
+    else if (mx == 3) NB_KP(false, 3);
     else NB_KP(false, 0);
 #undef NB_KP
     NB_LAUNCH_CHECK(ctx, "k_force_persistent");

@@ -119,19 +119,22 @@ __device__ __forceinline__ void pair_body(const double xi, const double yi, cons
     if (SNAP) A.sx = fma(w, tx, A.sx);
 }
 
-// The same pair in the paper's mixed precision (reading G27): the nine
+// The same pair in the paper's mixed precision (readings G27, G27b): the nine
 // differences are formed in double from the double records and rounded to float, everything
-// else of Eq. 8-10 is float arithmetic (FFMA/FMUL on the FP32 pipe, MUFU.RSQ), and the pair
-// terms are summed in float within one j-tile (the caller adds the tile sums in double).
-// FP64-pipe work per pair: 9 DADD + 10 F2F instead of 53 instructions.
+// else of Eq. 8-10 is float arithmetic (FFMA/FMUL on the FP32 pipe, MUFU.RSQ).
+//   ACC64 = false (reading G27, nb_set_precision 1): the pair terms are summed in float within one j-tile
+//     (the caller adds the tile sums in double).  FP64-pipe work per pair: 9 DADD + 10 F2F.
+//   ACC64 = true (reading G27b, nb_set_precision 2): the acceleration and jerk terms of every pair -- float
+//     products, rounded once -- are converted and ADDED IN DOUBLE (6 DP additions: with the 9 differences the
+//     15 double-precision operations PAPER.md:301 counts); the snap terms are summed in float as above.
 struct AccF {
     float ax, ay, az, jx, jy, jz, sx, sy, sz;
 };
-template <bool GUARD0>
+template <bool GUARD0, bool ACC64 = false>
 __device__ __forceinline__ void pair_body_mx(const double xi, const double yi, const double zi,
                                              const double vxi, const double vyi, const double vzi,
                                              const double axi, const double ayi, const double azi,
-                                             const double *__restrict__ q, const float eps2, AccF &A)
+                                             const double *__restrict__ q, const float eps2, AccF &A, Acc9 &D)
 {
     const double2 p0 = *reinterpret_cast<const double2 *>(q);
     const double2 p1 = *reinterpret_cast<const double2 *>(q + 2);
@@ -157,8 +160,13 @@ __device__ __forceinline__ void pair_body_mx(const double xi, const double yi, c
     const float b3 = fmaf(g * g, -1.0f / 3.0f, qq * vr);  // -3 beta
     const float g2 = g + g;
     const float ux = fmaf(g, dx, dvx), uy = fmaf(g, dy, dvy), uz = fmaf(g, dz, dvz);
-    A.ax = fmaf(w, dx, A.ax); A.ay = fmaf(w, dy, A.ay); A.az = fmaf(w, dz, A.az);
-    A.jx = fmaf(w, ux, A.jx); A.jy = fmaf(w, uy, A.jy); A.jz = fmaf(w, uz, A.jz);
+    if (ACC64) {
+        D.ax += (double)(w * dx); D.ay += (double)(w * dy); D.az += (double)(w * dz);
+        D.jx += (double)(w * ux); D.jy += (double)(w * uy); D.jz += (double)(w * uz);
+    } else {
+        A.ax = fmaf(w, dx, A.ax); A.ay = fmaf(w, dy, A.ay); A.az = fmaf(w, dz, A.az);
+        A.jx = fmaf(w, ux, A.jx); A.jy = fmaf(w, uy, A.jy); A.jz = fmaf(w, uz, A.jz);
+    }
     float tx = fmaf(g2, ux, dax), ty = fmaf(g2, uy, day), tz = fmaf(g2, uz, daz);
     tx = fmaf(b3, dx, tx); ty = fmaf(b3, dy, ty); tz = fmaf(b3, dz, tz);
     A.sx = fmaf(w, tx, A.sx); A.sy = fmaf(w, ty, A.sy); A.sz = fmaf(w, tz, A.sz);
@@ -208,7 +216,8 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 // (the paper shrinks its thread blocks instead).  `tc` counts the tiles this CTA has
 // consumed so far: ring stage = tc & 1, mbarrier phase = (tc >> 1) & 1, so the ring carries over
 // from item to item.
-// MX: 0 = FP64, 1 = mixed precision (reading G27), 2 = FP64 acceleration and jerk only
+// MX: 0 = FP64, 1 = mixed precision (reading G27), 2 = FP64 acceleration and jerk only,
+//     3 = mixed precision with acceleration and jerk accumulated in double (reading G27b)
 // The NT threads that work on an item are a whole CTA (VS = 0: tid = threadIdx.x, block barrier) or a
 // "virtual CTA" of NT threads on the named barrier `bar_id` inside a larger CTA (VS = 2, the resident
 // loop of nb_resident.cu).  The arithmetic and its order are the same.
@@ -272,14 +281,16 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
         mbar_wait(&full[sg], (tc >> 1) & 1u);
         if (!warp_idle) {
             const double *q = tile[sg] + jl * REC;
-            if (MX == 1) {
+            if (MX == 1 || MX == 3) {
                 AccF A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
                 const float eps2f = (float)eps2;
 #pragma unroll UNRM
                 for (int jj = 0; jj < PER; ++jj)
-                    pair_body_mx<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * (JL * REC), eps2f, A);
-                T.ax += (double)A.ax; T.ay += (double)A.ay; T.az += (double)A.az;
-                T.jx += (double)A.jx; T.jy += (double)A.jy; T.jz += (double)A.jz;
+                    pair_body_mx<GUARD0, MX == 3>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + jj * (JL * REC), eps2f, A, T);
+                if (MX == 1) {
+                    T.ax += (double)A.ax; T.ay += (double)A.ay; T.az += (double)A.az;
+                    T.jx += (double)A.jx; T.jy += (double)A.jy; T.jz += (double)A.jz;
+                }
                 T.sx += (double)A.sx; T.sy += (double)A.sy; T.sz += (double)A.sz;
             } else {
                 Acc9 A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
@@ -299,7 +310,7 @@ __device__ __forceinline__ void force_item(const double *__restrict__ jp, const 
         ++tc;
     }
 
-    if (MX != 1) {  // the FP64 pair body accumulates 3 sqrt(3) times the sums (pair_body)
+    if (MX == 0 || MX == 2) {  // the FP64 pair body accumulates 3 sqrt(3) times the sums (pair_body)
         T.ax *= PAIR_SCALE; T.ay *= PAIR_SCALE; T.az *= PAIR_SCALE;
         T.jx *= PAIR_SCALE; T.jy *= PAIR_SCALE; T.jz *= PAIR_SCALE;
         T.sx *= PAIR_SCALE; T.sy *= PAIR_SCALE; T.sz *= PAIR_SCALE;

@@ -92,16 +92,18 @@ __device__ __forceinline__ Acc9 res_eval(const double *ri, const double *rec, co
     Acc9 T = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     const double *q = rec + jl * REC;
     const int per = NL / JL;
-    if (MX == 1) {
+    if (MX == 1 || MX == 3) {
         const float eps2f = (float)eps2;
         for (int j0 = 0; j0 < per; j0 += 128) {        // float sums over at most 128 pair terms, as in force_item
             AccF A = {0, 0, 0, 0, 0, 0, 0, 0, 0};
             const int j1 = min(per, j0 + 128);
 #pragma unroll 4
             for (int jj = j0; jj < j1; ++jj)
-                pair_body_mx<GUARD0>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + (size_t)jj * (JL * REC), eps2f, A);
-            T.ax += (double)A.ax; T.ay += (double)A.ay; T.az += (double)A.az;
-            T.jx += (double)A.jx; T.jy += (double)A.jy; T.jz += (double)A.jz;
+                pair_body_mx<GUARD0, MX == 3>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + (size_t)jj * (JL * REC), eps2f, A, T);
+            if (MX == 1) {
+                T.ax += (double)A.ax; T.ay += (double)A.ay; T.az += (double)A.az;
+                T.jx += (double)A.jx; T.jy += (double)A.jy; T.jz += (double)A.jz;
+            }
             T.sx += (double)A.sx; T.sy += (double)A.sy; T.sz += (double)A.sz;
         }
     } else {
@@ -109,7 +111,7 @@ __device__ __forceinline__ Acc9 res_eval(const double *ri, const double *rec, co
         for (int jj = 0; jj < per; ++jj)
             pair_body<GUARD0, true>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + (size_t)jj * (JL * REC), eps2, T);
     }
-    if (MX != 1) {  // the FP64 pair body accumulates 3 sqrt(3) times the sums (pair_body)
+    if (MX == 0) {  // the FP64 pair body accumulates 3 sqrt(3) times the sums (pair_body)
         T.ax *= PAIR_SCALE; T.ay *= PAIR_SCALE; T.az *= PAIR_SCALE;
         T.jx *= PAIR_SCALE; T.jy *= PAIR_SCALE; T.jz *= PAIR_SCALE;
         T.sx *= PAIR_SCALE; T.sy *= PAIR_SCALE; T.sz *= PAIR_SCALE;
@@ -396,11 +398,13 @@ static cudaError_t launch_resident(nb_ctx *ctx, int n_cta)
 
 static cudaError_t launch_resident_any(nb_ctx *ctx, int n_cta)
 {
-    const bool mx = ctx->precision == 1;
+    const int mx = ctx->precision == 1 ? 1 : (ctx->precision == 2 ? 3 : 0);
     const bool g0 = mx ? (float)ctx->eps2 < 1e-24f : ctx->eps == 0.0;   // as in nb_force.cu
-    if (g0 && mx) return launch_resident<true, 1>(ctx, n_cta);
+    if (g0 && mx == 1) return launch_resident<true, 1>(ctx, n_cta);
+    if (g0 && mx == 3) return launch_resident<true, 3>(ctx, n_cta);
     if (g0) return launch_resident<true, 0>(ctx, n_cta);
-    if (mx) return launch_resident<false, 1>(ctx, n_cta);
+    if (mx == 1) return launch_resident<false, 1>(ctx, n_cta);
+    if (mx == 3) return launch_resident<false, 3>(ctx, n_cta);
     return launch_resident<false, 0>(ctx, n_cta);
 }
 

@@ -184,7 +184,7 @@ def run_fig1(nb, Ns, etas, t_end=4.5, every=0.5, eps=1e-4):
                          "pairs": st["n_pairs"] - 2.0 * N * N, "wall_s": wall})
             print(json.dumps(rows[-1]), file=sys.stderr, flush=True)
             g.close()
-    return {"experiment": "fig1_energy_vs_eta", "precision": "mixed" if PRECISION else "fp64", "eps": eps, "t_end": t_end, "sample_every": every, "rows": rows}
+    return {"experiment": "fig1_energy_vs_eta", "precision": ["fp64", "mixed", "mixed2"][PRECISION], "eps": eps, "t_end": t_end, "sample_every": every, "rows": rows}
 
 
 def run_probe(nb):
@@ -211,13 +211,14 @@ def main():
     ap.add_argument("--ms", default=None, help="comma-separated active-set sizes for --config 4 (default: the config's five)")
     ap.add_argument("--heavy-frac", type=float, default=0.05)
     ap.add_argument("--loop", type=int, default=None, choices=[0, 1, 2, 3], help="0: host-driven loop, 1: device-driven graph batches, 2: the same with programmatic dependent launch, 3: cluster-resident loop (N <= 16384); default: 3 for N <= 2048, else 1")
-    ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"],
-                    help="evaluation arithmetic: fp64 (default) or the paper's mixed SP/DP scheme (PAPER.md:287)")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed", "mixed2"],
+                    help="evaluation arithmetic: fp64 (default), the paper's mixed SP/DP scheme (PAPER.md:287, reading G27), "
+                         "or the same with acceleration and jerk summed in double (reading G27b: the 15 DP operations of PAPER.md:301)")
     a = ap.parse_args()
     import paper_1207_2367_b200 as nb
     from workloads import CONFIGS
     global PRECISION
-    PRECISION = 1 if a.precision == "mixed" else 0
+    PRECISION = {"fp64": 0, "mixed": 1, "mixed2": 2}[a.precision]
     if a.experiment == "splitj":
         N = a.n or (1 << 20)
         ms = [1, 2, 4, 8, 16, 32, 64, 128, 256, 1024, 4096, 16384, 65536, 262144]
