@@ -232,7 +232,7 @@ int nb_probe_fp64_peak(nb_ctx *ctx, int64_t iters, double *flops, float *ms);
 const char *nb_last_error(const nb_ctx *ctx);
 void nb_free(nb_ctx *ctx);
 
-/* Library version string, e.g. "nb-b200 0.2 (sm_100a)".                                     */
+/* Library version string, e.g. "nb-b200 0.3 (sm_100a)".                                     */
 const char *nb_version(void);
 
 #ifdef __cplusplus

@@ -48,7 +48,7 @@ static void release(nb_ctx *ctx)
     delete ctx;
 }
 
-extern "C" const char *nb_version(void) { return "nb-b200 0.2 (sm_100a)"; }
+extern "C" const char *nb_version(void) { return "nb-b200 0.3 (sm_100a)"; }
 
 extern "C" const char *nb_last_error(const nb_ctx *ctx) { return ctx ? ctx->err : "null context"; }
 

@@ -125,11 +125,11 @@ __global__ void k_unpack_f1(const double *__restrict__ f1, const size_t f1stride
 }
 
 // ---- host side ---------------------------------------------------------------------------
-// The split search never asks for more than MAX_WAVES waves of CTAs, i.e. S * n_ib <= MAX_WAVES x
-// (resident CTAs), each i-block of NT_E / JL >= 4 slots; S <= 65535 splits of mpad <= m + 31 add the slack term.
+// The split search never asks for more than MAX_WAVES work items per SM, i.e. S * n_ib <= MAX_WAVES x SMs items of
+// at most NT_E slots each; S <= 65535 splits of mpad <= m + 31 add the slack term.
 static size_t partials_bound(const nb_ctx *ctx)
 {
-    int64_t items = (int64_t)MAX_WAVES * ctx->n_sm * ctx->occ[0] * NT_E + 32 * 65536;
+    int64_t items = (int64_t)MAX_WAVES * ctx->n_sm * NT_E + 32 * 65536;
     const int64_t by_n = (ctx->Npad / TJ_E) * (ctx->Npad + 32);   // S <= tiles, mpad <= Npad + 32
     if (by_n < items) items = by_n;
     return (size_t)(9 * items);

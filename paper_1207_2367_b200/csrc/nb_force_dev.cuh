@@ -392,15 +392,27 @@ __device__ __forceinline__ double sum_splits_warp(const double *__restrict__ p, 
 }
 
 // All nine components of slot k, by one warp (all 32 lanes call it): f1[c][k] <- fixed-order sum over the splits.
+// For S >= 32 the nine lane-strided sums advance together, so that a lane has nine (unrolled: eighteen) independent
+// loads in flight instead of one component's at a time; per component the additions are those of sum_splits_warp,
+// in the same order.
 __device__ __forceinline__ void reduce_one(const double *__restrict__ part, const int S, const PartLayout &L, const int k,
                                            const int lane, double *__restrict__ f1, const int64_t Npad)
 {
     if (S < 32) {
         if (lane < 9) f1[lane * Npad + k] = sum_splits_thread(part + lane * L.cstride + (size_t)k * L.kstride, S, L.sstride);
     } else {
+        const double *p = part + (size_t)k * L.kstride;
+        double acc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+#pragma unroll 2
+        for (int s = lane; s < S; s += 32) {
+#pragma unroll
+            for (int cc = 0; cc < 9; ++cc) acc[cc] += p[cc * L.cstride + s];
+        }
+#pragma unroll
         for (int cc = 0; cc < 9; ++cc) {
-            const double acc = sum_splits_warp(part + cc * L.cstride + (size_t)k * L.kstride, S, lane);
-            if (lane == 0) f1[cc * Npad + k] = acc;
+            double a = acc[cc];
+            for (int off = 16; off > 0; off >>= 1) a += __shfl_xor_sync(0xffffffffu, a, off);
+            if (lane == 0) f1[cc * Npad + k] = a;
         }
     }
     __syncwarp();

@@ -85,17 +85,25 @@ constexpr int NT_E = 128, TJ_E = 128, MINB_E = 4;   // evaluation CTA: 128 threa
 constexpr int JL_MAX = 32;                           // at most one warp shares one i
 constexpr int64_t L2_CHUNK_BYTES = 24 << 20;         // j-stream piece kept L2-resident across i-block waves
 constexpr int GEOM_CACHE_M = 4096;                   // the device loop remembers the geometry of set sizes up to this
-constexpr int MAX_WAVES = 64;                       // the split search considers 1..MAX_WAVES waves
+constexpr int MAX_WAVES = 255;                      // the split search considers 1..MAX_WAVES work items per SM
 constexpr int64_t RES_MAX_N = 2048;                  // the cluster-resident loop (nb_resident.cu) keeps N up to this on chip
 constexpr int64_t RES_AUTO_N = 2048;                 // ... and is the default driver up to this
 
-// Number of j-splits.  All CTAs do the same work per tile, so the cost of a launch is
-// waves x (tiles per split + a fixed per-CTA cost of 0.75 tile) + 0.002 S, in integer
-// thousandths so that host and device take the identical decision.  For a given number of
-// waves w the best S is the largest that still fits, so only the candidates w = 0..MAX_WAVES
-// are scored (w = 0 stands for S = 1); the first candidate with the least cost wins.
+// Number of j-splits.  The evaluation is bound by the FP64 pipe of the SM, which the CTAs resident on an SM
+// share: what a launch costs is the work of the most loaded SM, (work items on it) x (tiles per item + a
+// fixed 0.15 tile per item), in integer thousandths so that host and device take the identical decision.
+// Items are handed out one by one (block scheduler / the work counter of the persistent kernel), so the most
+// loaded SM holds ceil(items / SMs) of them.  (Round 1 counted waves of SMs x resident CTAs: 683 CTAs on
+// 148 SMs x 5 are "one wave", but 91 SMs hold five items and 57 four -- 8 % lost; measured at N = 2^20,
+// m = 128: 497 us with 683 splits of 12 tiles, 453 us with 2048 splits of 4.)  Half an item is added for the
+// ramp-up and the tail of a launch, which shorter items shrink.  An SM needs about four
+// resident CTAs (4 warps per sub-partition) to cover the DFMA latency: fewer items per SM are charged
+// in proportion.  0.002 S accounts for the partial sums (0.004, 0.008 S when 16, 32 lanes share an i: a tile is
+// then 8, 4 pairs per thread, and m <= 4 is bound by HBM, not by the pipe: measured best 586 splits at m = 1, 1171 at m >= 8).  For w items per SM the best S is the largest that
+// still fits, so only the candidates w = 0..MAX_WAVES are scored (w = 0 stands for S = 1); the first candidate
+// with the least cost wins.
 struct SplitProblem {
-    int64_t n_ib, tiles, slots, s_cap;
+    int64_t n_ib, tiles, slots, s_cap, n_sm, jl;
 };
 // candidate w -> its S; returns the cost, or INT64_MAX when the candidate does not exist
 __host__ __device__ inline int64_t split_candidate(const SplitProblem &p, int64_t w, int *S_out)
@@ -104,14 +112,17 @@ __host__ __device__ inline int64_t split_candidate(const SplitProblem &p, int64_
     if (s_cap > p.tiles) s_cap = p.tiles;
     if (s_cap > 65535) s_cap = 65535;
     if (s_cap < 1) s_cap = 1;
-    int64_t S = (w == 0) ? 1 : (w * p.slots) / p.n_ib;
+    int64_t S = (w == 0) ? 1 : (w * p.n_sm) / p.n_ib;
     if (S < 1) { *S_out = 1; return INT64_MAX; }
     if (S > s_cap) S = s_cap;
     const int64_t tps = (p.tiles + S - 1) / S;
     S = (p.tiles + tps - 1) / tps;  // splits that actually get tiles
-    const int64_t waves = (p.n_ib * S + p.slots - 1) / p.slots;
+    const int64_t per_sm = (p.n_ib * S + p.n_sm - 1) / p.n_sm;   // items on the most loaded SM
+    int64_t cost = per_sm * (tps * 1000 + 150) + 500 * tps;      // + half an item of ramp-up / tail
+    const int64_t want = p.slots / p.n_sm < 4 ? p.slots / p.n_sm : 4;
+    if (per_sm < want) cost = cost * want / per_sm;              // too few warps to keep the FP64 pipe busy
     *S_out = (int)S;
-    return waves * (tps * 1000 + 750) + 2 * S;
+    return cost + S * (p.jl > 8 ? p.jl / 4 : 2);                 // the partial sums; dearer against the short tiles of many lanes per i
 }
 __host__ __device__ inline int choose_split(const SplitProblem &p)
 {
@@ -140,6 +151,8 @@ __host__ __device__ inline SplitProblem geom_begin(ForceGeom &g, int64_t m, int6
     p.n_ib = (m + slots_per_cta - 1) / slots_per_cta;
     p.tiles = Npad / TJ_E;
     p.slots = (int64_t)n_sm * occ;
+    p.n_sm = n_sm;
+    p.jl = JL;
     const int64_t mpad = (m + 31) & ~(int64_t)31;
     p.s_cap = partials_cap / (9 * mpad);
     g.JL = JL; g.n_ib = (int)p.n_ib; g.mpad = (int)mpad; g.pad_ = 0;
