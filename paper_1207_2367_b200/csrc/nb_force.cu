@@ -50,8 +50,30 @@ __global__ void __launch_bounds__(NT_E, MINB_E)
 // from a counter in the control block (items of one launch take equally long, but CTAs do not start
 // together: a fixed stride left a 2 % tail at m ~ 2e5).  Item w is (i-block w % n_ib, split
 // w / n_ib), so concurrently running CTAs stream the same j-split.
+// The lane count of a step is known only on the device, so the kernel holds all six force_item instantiations.
+// Inlined into one body they share one register allocation (122 registers: a fifth of the warps lost, and a cap of
+// 96 costs the pair loop its operand-reuse order).  So only the throughput path (one i per lane) is inline; the five
+// lane-sharing instantiations of the small sets are NON-INLINED device functions with their own allocation.  They find
+// the tile ring in the dynamic shared memory of the kernel, so their loads stay LDS.
+constexpr size_t PERSIST_RING = 2 * TJ_E * REC * sizeof(double);
+constexpr size_t PERSIST_SMEM = PERSIST_RING + 2 * sizeof(uint64_t) + sizeof(long long);
+
+template <int JL, bool GUARD0, int MX, int UNR>
+__device__ __noinline__ unsigned persistent_item(const double *__restrict__ jp, const int32_t *__restrict__ active, const int m,
+                                                 const int ib, const int sp, const int tiles_total, const int tps,
+                                                 const double eps2, double *__restrict__ out, const size_t cstride,
+                                                 const size_t kstride, const size_t sstride, unsigned tc)
+{
+    extern __shared__ __align__(128) unsigned char persist_smem[];
+    double (*tile)[TJ_E * REC] = reinterpret_cast<double (*)[TJ_E * REC]>(persist_smem);
+    uint64_t *full = reinterpret_cast<uint64_t *>(persist_smem + PERSIST_RING);
+    force_item<NT_E, TJ_E, JL, GUARD0, MX, UNR>(jp, jp, active, m, ib, sp, tiles_total, tps, eps2, out, cstride, kstride,
+                                                sstride, tile, full, tc);
+    return tc;
+}
+
 template <bool GUARD0, int MX = 0, int UNR = 12>
-__global__ void __launch_bounds__(NT_E, MINB_E)
+__global__ void __launch_bounds__(NT_E, 5)
     k_force_persistent(const double *__restrict__ jp, const int32_t *__restrict__ active_list, const int64_t N,
                        const int64_t Npad, const double eps2, double *__restrict__ f1,
                        double *__restrict__ partials, StepCtl *__restrict__ ctl)
@@ -59,9 +81,9 @@ __global__ void __launch_bounds__(NT_E, MINB_E)
     pdl_trigger();
     pdl_wait();
     if (ctl->done) return;
-    __shared__ __align__(128) double tile[2][TJ_E * REC];
-    __shared__ __align__(8) uint64_t full[2];
-    __shared__ long long next_item;
+    extern __shared__ __align__(128) unsigned char persist_smem[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(persist_smem + PERSIST_RING);
+    long long *next_item = reinterpret_cast<long long *>(persist_smem + PERSIST_RING + 2 * sizeof(uint64_t));
     if (threadIdx.x == 0) {
         mbar_init(&full[0], 1);
         mbar_init(&full[1], 1);
@@ -78,11 +100,24 @@ __global__ void __launch_bounds__(NT_E, MINB_E)
     unsigned tc = 0;
     long long w = blockIdx.x;
     while (w < items) {
-        force_item_jl<NT_E, TJ_E, GUARD0, MX, UNR>(g.JL, jp, jp, active, m, (int)(w % g.n_ib), (int)(w / g.n_ib), tiles_total,
-                                                   g.tps, eps2, out, L.cstride, L.kstride, L.sstride, tile, full, tc);
-        if (threadIdx.x == 0) next_item = (long long)gridDim.x + atomicAdd(&ctl->work, 1u);
+        const int ib = (int)(w % g.n_ib), sp = (int)(w / g.n_ib);
+#define NB_PI(J) tc = persistent_item<J, GUARD0, MX, UNR>(jp, active, m, ib, sp, tiles_total, g.tps, eps2, out, L.cstride, L.kstride, L.sstride, tc)
+        switch (g.JL) {
+            case 1:   // the throughput path stays inline: its pair loop keeps the schedule of k_force<1>
+                force_item<NT_E, TJ_E, 1, GUARD0, MX, UNR>(jp, jp, active, m, ib, sp, tiles_total, g.tps, eps2, out, L.cstride,
+                                                           L.kstride, L.sstride, reinterpret_cast<double (*)[TJ_E * REC]>(persist_smem),
+                                                           full, tc);
+                break;
+            case 2: NB_PI(2); break;
+            case 4: NB_PI(4); break;
+            case 8: NB_PI(8); break;
+            case 16: NB_PI(16); break;
+            default: NB_PI(32); break;
+        }
+#undef NB_PI
+        if (threadIdx.x == 0) *next_item = (long long)gridDim.x + atomicAdd(&ctl->work, 1u);
         __syncthreads();
-        w = next_item;
+        w = *next_item;
         __syncthreads();
     }
 }
@@ -140,7 +175,7 @@ int query_force_occupancy(nb_ctx *ctx)
     int v = 0;
     NB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_force<1, false>, NT_E, 0));
     ctx->occ[0] = v > 0 ? v : 1;
-    NB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_force_persistent<false>, NT_E, 0));
+    NB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_force_persistent<false>, NT_E, PERSIST_SMEM));
     ctx->occ[1] = v > 0 ? v : 1;
     ctx->partials_limit = partials_bound(ctx);
     return NB_OK;
@@ -231,7 +266,7 @@ int enqueue_force_persistent(nb_ctx *ctx)
 {
     const unsigned gP = (unsigned)(ctx->n_sm * ctx->occ[1]);
 #define NB_KP(G0, MXP)                                                                                      \
-    launch_chain(k_force_persistent<G0, MXP>, dim3(gP), dim3(NT_E), ctx->stream, pdl, ctx->jp, ctx->active, \
+    launch_chain(k_force_persistent<G0, MXP>, dim3(gP), dim3(NT_E), ctx->stream, pdl, PERSIST_SMEM, ctx->jp, ctx->active, \
                  ctx->N, ctx->Npad, ctx->eps2, ctx->f1, ctx->partials, ctx->ctl)
     const int mx = ctx->precision == 1 ? 1 : (ctx->precision == 2 ? 3 : 0);
     const bool pdl = ctx->use_graph == 2;

@@ -609,7 +609,7 @@ int launch_graph_begin(nb_ctx *ctx, double t_end, int64_t steps)
 int enqueue_graph_gather_predict(nb_ctx *ctx, int parity)
 {
     const unsigned np = (unsigned)((ctx->N + SCHED_THREADS - 1) / SCHED_THREADS);
-    launch_chain(k_g_gather_predict, dim3(np), dim3(SCHED_THREADS), ctx->stream, ctx->use_graph == 2, parity, ctx->N,
+    launch_chain(k_g_gather_predict, dim3(np), dim3(SCHED_THREADS), ctx->stream, ctx->use_graph == 2, (size_t)0, parity, ctx->N,
                  ctx->Npad, ctx->t, ctx->dt, ctx->active, ctx->ctl, ctx->mass, ctx->r, ctx->v, ctx->a, ctx->j, ctx->s,
                  ctx->c, ctx->jp, ctx->n_sm, ctx->occ[0], (int64_t)ctx->partials_limit, ctx->force_split,
                  ctx->force_jlanes, ctx->geom_cache);
@@ -622,7 +622,7 @@ int enqueue_graph_correct(nb_ctx *ctx, int parity)
     // enough warps for one per active particle of a small set; large sets (one split) go thread per particle
     int64_t g = (ctx->N + SCHED_THREADS - 1) / SCHED_THREADS;
     if (g > 4 * ctx->n_sm) g = 4 * ctx->n_sm;
-    launch_chain(k_g_reduce_correct, dim3((unsigned)g), dim3(SCHED_THREADS), ctx->stream, ctx->use_graph == 2, parity, ctx->N,
+    launch_chain(k_g_reduce_correct, dim3((unsigned)g), dim3(SCHED_THREADS), ctx->stream, ctx->use_graph == 2, (size_t)0, parity, ctx->N,
                  ctx->Npad, ctx->active, ctx->ctl, ctx->eta, ctx->dt_min, ctx->dt_max, ctx->partials, ctx->f1, ctx->t, ctx->dt,
                  ctx->r, ctx->v, ctx->a, ctx->j, ctx->s, ctx->c);
     NB_LAUNCH_CHECK(ctx, "k_g_reduce_correct");
