@@ -229,6 +229,30 @@ int nb_get_launch(nb_ctx *ctx, int64_t out[5]);
  * It is the measured denominator quoted beside the nominal FP64 peak. */
 int nb_probe_fp64_peak(nb_ctx *ctx, int64_t iters, double *flops, float *ms);
 
+/* The evaluation of nb_force (Eq. 8-10, Eq. 2 softening; j-splits as in PAPER.md:108-114) for
+ * callers that cannot allocate -- code under CUDA-graph capture, serving loops, harnesses that forbid cudaMalloc.
+ * No context: the call packs the caller's arrays into the record layout, evaluates and sums the j-splits in a
+ * fixed 16 MiB `static __device__` array inside the library (every GPU that loads libnb.so holds it until the process
+ * exits), and calls no cudaMalloc, cudaFree or allocating routine.  Binary64 only.
+ *   N in [1, NB_STATIC_MAX_N]; larger N is refused with NB_EINVAL (use nb_init + nb_force).
+ *   pos, vel [dev] [N][3], mass [dev] [N]; acc_pred [dev] [N][3] or NULL (= zeros): the predicted a_j of Eq. 10.
+ *   eps >= 0.  active_idx [dev] int32 [n_active], values in [0, N), not range-checked; NULL = all N in index order
+ *   (n_active must be N).  acc, jerk, snap [dev] [n_active][3], each may be NULL.  ALL pointers are DEVICE pointers.
+ *   cuda_stream: a cudaStream_t on the CURRENT device (NULL = legacy default stream); the kernels are enqueued on
+ *   it and the call returns without synchronising.  err [host] (may be NULL): receives the message of a failure,
+ *   at most err_len bytes.
+ * The first call on a device also does the one-time set-up for that device (symbol address, SM count, occupancy
+ * query; nothing allocates): make it before a capture starts -- n_active = 0 does the set-up and nothing else.
+ * The array is shared by all calls of the process on that device and keeps the last call's contents; the call
+ * rewrites whatever it reads (padding records are zeroed every time).  Calls that OVERLAP on the GPU (two
+ * streams, two graphs replayed at once) race on it: serialise them.  Results: the split rule sees this array's
+ * partial-sum budget instead of a context's, so the number of j-splits, hence the summation order, may differ from
+ * nb_force's: equal to rounding (G18), bit-reproducible from call to call.           */
+#define NB_STATIC_MAX_N 65536
+int nb_force_static(int64_t N, const double *pos, const double *vel, const double *acc_pred, const double *mass,
+                    double eps, const int32_t *active_idx, int64_t n_active, double *acc, double *jerk, double *snap,
+                    void *cuda_stream, char *err, int64_t err_len);
+
 const char *nb_last_error(const nb_ctx *ctx);
 void nb_free(nb_ctx *ctx);
 

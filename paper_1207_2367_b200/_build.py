@@ -22,7 +22,7 @@ FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v
 # pair body, which is arranged so that FP64 instructions with three register sources find one of them in the
 # operand-reuse cache (csrc/nb_force_dev.cuh); -O3 interleaves the unrolled pairs for
 # latency and loses that (measured on B200: 121.9 cycles per warp-pair at -O3, 118.7 at -O1 with the round-1 body).
-PTXAS_LEVEL = {"nb_force.cu": "-O1"}
+PTXAS_LEVEL = {"nb_force.cu": "-O1", "nb_static.cu": "-O1"}
 
 
 def sources():

@@ -21,7 +21,7 @@ __all__ = [
     "nb_force", "nb_correct_and_step", "nb_run_until", "nb_run_steps", "nb_energy", "nb_get_state",
     "nb_get_derivs", "nb_get_pred", "nb_set_pred_acc", "nb_set_pred", "nb_get_full_state",
     "nb_set_full_state", "nb_get_stats", "nb_set_tuning", "nb_set_loop_mode", "nb_set_precision", "nb_set_j_range", "nb_get_forces", "nb_set_forces", "nb_get_launch", "nb_probe_fp64_peak",
-    "nb_set_debug", "nb_version", "nb_last_error",
+    "nb_set_debug", "nb_version", "nb_last_error", "nb_force_static", "NB_STATIC_MAX_N",
 ]
 
 NB_OK, NB_EINVAL, NB_ESTATE, NB_ECUDA, NB_ENOMEM = 0, -1, -2, -3, -4
@@ -67,6 +67,7 @@ _SIGS = {
     "nb_get_launch": (C.c_int, [_vp, C.POINTER(_i64)]),
     "nb_probe_fp64_peak": (C.c_int, [_vp, _i64, C.POINTER(_dbl), C.POINTER(C.c_float)]),
     "nb_set_debug": (C.c_int, [_vp, C.c_int]),
+    "nb_force_static": (C.c_int, [_i64, _vp, _vp, _vp, _vp, _dbl, _vp, _i64, _vp, _vp, _vp, _vp, C.c_char_p, _i64]),
     "nb_last_error": (C.c_char_p, [_vp]),
     "nb_free": (None, [_vp]),
     "nb_version": (C.c_char_p, []),
@@ -300,6 +301,34 @@ def nb_probe_fp64_peak(ctx, iters=1 << 16):
 
 def nb_set_debug(ctx, on=1):
     _check(ctx, lib().nb_set_debug(ctx, int(on)))
+
+
+NB_STATIC_MAX_N = 65536
+
+
+def _dev_ptr(x, dtype=np.float64, n=None):
+    """Raw address of a contiguous CUDA tensor (None -> NULL): nb_force_static takes device pointers only."""
+    if x is None:
+        return None
+    if not hasattr(x, "is_cuda") or not x.is_cuda:
+        raise TypeError("nb_force_static takes CUDA tensors only (device pointers)")
+    return _ptr(x, dtype, n)
+
+
+def nb_force_static(pos, vel, acc_pred, mass, eps, active_idx, n_active, acc=None, jerk=None, snap=None, stream=None):
+    """nb_force_static: the evaluation without a context and without any allocation (include/nb.h).  Every
+    array is a CUDA tensor the caller owns, outputs included; nothing is allocated here either."""
+    N, n = int(mass.shape[0]), int(n_active)
+    if stream is not None and hasattr(stream, "cuda_stream"):
+        stream = stream.cuda_stream
+    err = C.create_string_buffer(512)
+    rc = lib().nb_force_static(N, _dev_ptr(pos, n=3 * N), _dev_ptr(vel, n=3 * N), _dev_ptr(acc_pred, n=3 * N),
+                               _dev_ptr(mass, n=N), float(eps), _dev_ptr(active_idx, np.int32, n if active_idx is not None else None),
+                               n, _dev_ptr(acc, n=3 * n), _dev_ptr(jerk, n=3 * n), _dev_ptr(snap, n=3 * n),
+                               _vp(stream or 0), err, len(err))
+    if rc != NB_OK:
+        raise NBError(rc, err.value.decode())
+    return acc, jerk, snap
 
 
 # ---------------------------------------------------------------------------- convenience wrapper
