@@ -393,6 +393,11 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+LOOP_NAMES = {0: "host-issued calls", 1: "device-driven CUDA-graph batches", 2: "CUDA-graph batches with programmatic dependent launch",
+              3: "cluster-resident loop (one kernel for the whole run, state in the shared memory of one cluster)",
+              4: "grid-resident loop (one cooperative kernel on all SMs, state in shared memory; large steps by the streaming kernels)"}
+
+
 def block_step_wall_time(nb, dev):
     """Wall time per block step of the Hermite loop (nb_run_until, device-driven) on the seeded inputs of
     BASELINE.json configs[0] (whole run) and configs[1] (first dt_max = 1/16 time unit)."""
@@ -405,9 +410,8 @@ def block_step_wall_time(nb, dev):
         g = nb.NBody(dev(pos), dev(vel), dev(m), c["eps"], c["eta"], dt_min=c["dt_min"], dt_max=c["dt_max"])
         g.startup(); g.sync()
         e0 = g.energy()
-        loop = "cluster-resident loop (one kernel for the whole run, state in shared memory)" if c["N"] <= 2048 \
-            else "device-driven CUDA-graph batches"   # the library's default driver for this N (include/nb.h)
-        g.run_until(0.0)                       # builds the CUDA graph of this context outside the timed part
+        loop = LOOP_NAMES[nb.nb_get_loop_mode(g.ctx)]   # the library's default driver for this N (include/nb.h)
+        g.run_until(0.0)                       # first launch (graph capture, buffers) outside the timed part
         torch.cuda.synchronize()
         t0 = time.perf_counter(); n = g.run_until(t_end); torch.cuda.synchronize(); wall = time.perf_counter() - t0
         e1 = g.energy()

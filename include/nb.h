@@ -206,7 +206,7 @@ int nb_set_precision(nb_ctx *ctx, int mode);
  * returns NB_EINVAL instead of reading out of bounds; 0 (default) = no check, no cost.       */
 int nb_set_debug(nb_ctx *ctx, int on);
 
-/* Driver of nb_run_until / nb_run_steps (all give bit-identical states):
+/* Driver of nb_run_until / nb_run_steps:
  *   0  the host issues nb_next_block / nb_predict / nb_force / nb_correct_and_step per step;
  *   1  device-driven CUDA-graph batches (kernels read (t_next, n_active) from device memory);
  *   2  the same graph with its kernels chained by programmatic dependent launch (measured slower than
@@ -214,11 +214,21 @@ int nb_set_debug(nb_ctx *ctx, int on);
  *   3  ONE kernel resident on one thread-block cluster (up to 16 SMs) keeps the whole system in shared
  *      memory and runs every step, its phases separated by the hardware cluster barrier: no launch, no host
  *      round trip and no trip to L2 per step (the small blocks).  Serves N <= 2048 (NB_EINVAL
- *      above).  It adds the pair terms of a particle in its own fixed order (per owner CTA, then over the CTAs),
- *      so its results agree with modes 0-2 to rounding, not bit for bit (any order is correct, G18).
- * Modes 0, 1, 2 give bit-identical states.  Default: 3 for N <= 2048, else 1.  nb_run_steps with a per-step
- * log always uses 0.                                                                         */
+ *      above).
+ *   4  ONE cooperative kernel on ALL SMs, one CTA per SM, each keeping its share of the particles (state and
+ *      predicted records) in shared memory; a block step costs two grid barriers and a few reads of small
+ *      L2-resident buffers instead of three kernels.  Serves N up to 704 particles per SM (104 192 on a B200;
+ *      NB_EINVAL above).  Block steps with 2048 or more active particles are handed, one at a time, to the
+ *      call sequence of mode 0 (the streaming evaluation kernel at full occupancy) and the kernel is launched again.
+ * Modes 0, 1, 2 give bit-identical states.  Modes 3 and 4 add the pair terms of a particle in their own fixed order
+ * (per owner CTA, then over the CTAs), so their results agree with modes 0-2 to rounding, not bit for bit (any order
+ * is correct, G18), and are bit-reproducible from run to run.
+ * Default: 3 for N <= 2048, 4 while the system fits the shared memory of the device, else 1.  nb_run_steps with a
+ * per-step log always uses 0.                                                                 */
 int nb_set_loop_mode(nb_ctx *ctx, int device_driven);
+
+/* The driver nb_run_until / nb_run_steps will use on this context (0..4, as above) -> *mode [host].          */
+int nb_get_loop_mode(nb_ctx *ctx, int *mode);
 
 /* What the last nb_force launched: out [host] = {threads per CTA, j-lanes per i, j-splits,
  * CTAs, j-tile length}.                                                                     */

@@ -35,6 +35,7 @@ static void release(nb_ctx *ctx)
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
     graph_release(ctx);
+    gridres_release(ctx);
     if (ctx->h_ctl) cudaFreeHost(ctx->h_ctl);
     if (ctx->ctl) cudaFree(ctx->ctl);
     if (ctx->geom_cache) cudaFree(ctx->geom_cache);
@@ -139,7 +140,7 @@ extern "C" int nb_init(nb_ctx **out, int64_t N, const double *pos, const double 
         return fail(rc);
     if (cudaHostAlloc((void **)&ctx->h_ctl, sizeof(StepCtl), cudaHostAllocDefault) != cudaSuccess) return fail(NB_ENOMEM);
     memset(ctx->h_ctl, 0, sizeof(StepCtl));
-    ctx->use_graph = N <= RES_AUTO_N ? 3 : 1;
+    ctx->use_graph = N <= RES_AUTO_N ? 3 : (gridres_fits(ctx) ? 4 : 1);
     ctx->loop_auto = true;
     ctx->j_begin = 0; ctx->j_end = N;
     if ((rc = query_force_occupancy(ctx))) return fail(rc);
@@ -305,6 +306,16 @@ static int one_block_step(nb_ctx *ctx)
     return nb_correct_and_step(ctx);
 }
 
+int nb::host_block_step(nb_ctx *ctx, double t_end, bool *stepped)
+{
+    *stepped = false;
+    if (!ctx->have_block) NB_TRY(nb_next_block(ctx, nullptr, nullptr));
+    if (ctx->t_next > t_end) return NB_OK;
+    NB_TRY(one_block_step(ctx));
+    *stepped = true;
+    return NB_OK;
+}
+
 extern "C" int nb_run_until(nb_ctx *ctx, double t_end, int64_t *n_steps)
 {
     if (!ctx) return NB_EINVAL;
@@ -313,6 +324,7 @@ extern "C" int nb_run_until(nb_ctx *ctx, double t_end, int64_t *n_steps)
         return set_err(ctx, NB_ESTATE, "nb_run_until: a j-shard is set (nb_set_j_range); drive the steps call by call and all-reduce nb_get_forces");
     if (!ctx->started) NB_TRY(nb_startup(ctx));
     if (ctx->use_graph == 3) return resident_run(ctx, t_end, INT64_MAX, n_steps);
+    if (ctx->use_graph == 4) return gridres_run(ctx, t_end, INT64_MAX, n_steps);
     if (ctx->use_graph) return graph_run(ctx, t_end, INT64_MAX, n_steps);
     int64_t n = 0;
     for (;;) {
@@ -334,6 +346,7 @@ extern "C" int nb_run_steps(nb_ctx *ctx, int64_t n, double *log_t, int64_t *log_
     if (ctx->use_graph && !log_t && !log_m && !log_ms) {
         if (n == 0) return NB_OK;
         if (ctx->use_graph == 3) return resident_run(ctx, bits_to_double(0x7fefffffffffffffLL), n, nullptr);
+        if (ctx->use_graph == 4) return gridres_run(ctx, bits_to_double(0x7fefffffffffffffLL), n, nullptr);
         return graph_run(ctx, bits_to_double(0x7fefffffffffffffLL), n, nullptr);
     }
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -526,11 +539,20 @@ extern "C" int nb_set_precision(nb_ctx *ctx, int mode)
 extern "C" int nb_set_loop_mode(nb_ctx *ctx, int device_driven)
 {
     if (!ctx) return NB_EINVAL;
-    if (device_driven < 0 || device_driven > 3) return set_err(ctx, NB_EINVAL, "nb_set_loop_mode: 0, 1, 2 or 3");
+    if (device_driven < 0 || device_driven > 4) return set_err(ctx, NB_EINVAL, "nb_set_loop_mode: 0, 1, 2, 3 or 4");
+    if (device_driven == 4 && !gridres_fits(ctx))
+        return set_err(ctx, NB_EINVAL, "nb_set_loop_mode: mode 4 (grid-resident loop) does not hold N = %lld in the shared memory of this device", (long long)ctx->N);
     if (device_driven == 3 && ctx->N > RES_MAX_N)
         return set_err(ctx, NB_EINVAL, "nb_set_loop_mode: mode 3 (cluster-resident loop) serves N <= %lld", (long long)RES_MAX_N);
     ctx->use_graph = device_driven;
     ctx->loop_auto = false;
+    return NB_OK;
+}
+
+extern "C" int nb_get_loop_mode(nb_ctx *ctx, int *mode)
+{
+    if (!ctx || !mode) return NB_EINVAL;
+    *mode = ctx->use_graph;
     return NB_OK;
 }
 

@@ -88,6 +88,8 @@ constexpr int GEOM_CACHE_M = 4096;                   // the device loop remember
 constexpr int MAX_WAVES = 255;                      // the split search considers 1..MAX_WAVES work items per SM
 constexpr int64_t RES_MAX_N = 2048;                  // the cluster-resident loop (nb_resident.cu) keeps N up to this on chip
 constexpr int64_t RES_AUTO_N = 2048;                 // ... and is the default driver up to this
+constexpr int GR_M_BIG_DEFAULT = 2048;               // grid-resident loop (nb_gridres.cu): steps with this many active particles
+                                                     // or more go to the streaming kernels
 
 // Number of j-splits.  The evaluation is bound by the FP64 pipe of the SM, which the CTAs resident on an SM
 // share: what a launch costs is the work of the most loaded SM, (work items on it) x (tiles per item + a
@@ -234,6 +236,10 @@ struct nb_ctx {
     int res_cluster;                // CTAs of the resident loop's cluster (16, or 8 where 16 cannot be scheduled)
     bool loop_auto;                 // the loop mode is the default for this N (not set by nb_set_loop_mode)
     int graph_pdl;                  // the captured graph uses programmatic dependent launch
+    void *gr_hdr;                   // grid-resident loop (nb_gridres.cu): per-CTA headers, candidates' records, partial sums,
+    double *gr_cand, *gr_part;      // barrier counter; allocated at the first run in loop mode 4
+    unsigned long long *gr_bar;
+    int gr_m_big, gr_m_big_alloc;
 
     // tuning
     int force_split, force_jlanes;
@@ -290,6 +296,11 @@ void graph_release(nb_ctx *ctx);
 // ----- nb_resident.cu
 int resident_run(nb_ctx *ctx, double t_end, int64_t max_steps, int64_t *n_steps);
 
+// ----- nb_gridres.cu
+int gridres_run(nb_ctx *ctx, double t_end, int64_t max_steps, int64_t *n_steps);
+bool gridres_fits(const nb_ctx *ctx);
+void gridres_release(nb_ctx *ctx);
+
 // ----- nb_energy.cu
 int launch_energy(nb_ctx *ctx, const double *records, double out_host[9]);
 
@@ -298,6 +309,8 @@ int launch_probe(nb_ctx *ctx, int64_t iters, double *flops, float *ms);
 
 // ----- nb_api.cu
 int reserve_stage(nb_ctx *ctx, size_t doubles);
+// one block step through the call sequence (next block [sync], predict, evaluate, correct) unless the next block lies beyond t_end
+int host_block_step(nb_ctx *ctx, double t_end, bool *stepped);
 
 int set_err(nb_ctx *ctx, int code, const char *fmt, ...);
 

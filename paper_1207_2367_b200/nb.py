@@ -20,7 +20,7 @@ __all__ = [
     "nb_init", "nb_free", "nb_set_limits", "nb_startup", "nb_startup_commit", "nb_next_block", "nb_get_active", "nb_predict",
     "nb_force", "nb_correct_and_step", "nb_run_until", "nb_run_steps", "nb_energy", "nb_get_state",
     "nb_get_derivs", "nb_get_pred", "nb_set_pred_acc", "nb_set_pred", "nb_get_full_state",
-    "nb_set_full_state", "nb_get_stats", "nb_set_tuning", "nb_set_loop_mode", "nb_set_precision", "nb_set_j_range", "nb_get_forces", "nb_set_forces", "nb_get_launch", "nb_probe_fp64_peak",
+    "nb_set_full_state", "nb_get_stats", "nb_set_tuning", "nb_set_loop_mode", "nb_get_loop_mode", "nb_set_precision", "nb_set_j_range", "nb_get_forces", "nb_set_forces", "nb_get_launch", "nb_probe_fp64_peak",
     "nb_set_debug", "nb_version", "nb_last_error", "nb_force_static", "NB_STATIC_MAX_N",
 ]
 
@@ -60,6 +60,7 @@ _SIGS = {
     "nb_get_stats": (C.c_int, [_vp, C.POINTER(_dbl), C.POINTER(_i64)]),
     "nb_set_tuning": (C.c_int, [_vp, C.c_int, C.c_int]),
     "nb_set_loop_mode": (C.c_int, [_vp, C.c_int]),
+    "nb_get_loop_mode": (C.c_int, [_vp, C.POINTER(C.c_int)]),
     "nb_set_precision": (C.c_int, [_vp, C.c_int]),
     "nb_set_j_range": (C.c_int, [_vp, _i64, _i64]),
     "nb_get_forces": (C.c_int, [_vp, _vp]),
@@ -268,6 +269,12 @@ def nb_set_tuning(ctx, split=0, jlanes=0):
 
 def nb_set_loop_mode(ctx, device_driven=1):
     _check(ctx, lib().nb_set_loop_mode(ctx, int(device_driven)))
+
+
+def nb_get_loop_mode(ctx) -> int:
+    mode = C.c_int()
+    _check(ctx, lib().nb_get_loop_mode(ctx, C.byref(mode)))
+    return mode.value
 
 
 def nb_set_precision(ctx, mode=0):

@@ -1,11 +1,12 @@
 """The device-driven block-step loops (CUDA-graph batches, csrc/nb_graph.cu; the cluster-resident
-loop, csrc/nb_resident.cu) against the host-driven call sequence nb_next_block -> nb_predict ->
+loop, csrc/nb_resident.cu; the grid-resident loop, csrc/nb_gridres.cu) against the host-driven call sequence nb_next_block -> nb_predict ->
 nb_force -> nb_correct_and_step.
 
 The graph-driven loop (modes 1, 2) runs the same device functions with the same geometry rule and the
 same summation order as the call sequence, so the committed state must be BIT-identical: positions,
 velocities, derivatives, times, time steps, step count, pair count and the histogram of active-set
-sizes.  The cluster-resident loop (mode 3) adds the pair terms of a particle in its own fixed order
+sizes.  The cluster-resident loop (mode 3) and the grid-resident loop (mode 4: all SMs, two grid barriers per
+step, large steps handed to the call sequence) add the pair terms of a particle in their own fixed order
 (G18: any order is correct), so it must reproduce times, time steps, step and pair counts
 exactly and everything else to rounding (1e-12 of the particle's own magnitude), and be bit-reproducible
 from run to run.  Parity of the
@@ -22,9 +23,13 @@ from workloads import kepler_binary, plummer
 pytestmark = pytest.mark.gpu
 
 
+OWN_ORDER = (3, 4)   # loop modes with their own summation order
+
+
 def _mk(nb, pos, vel, m, eps, eta, dt_min, dt_max, graph):
     """graph: False/0 = host-issued calls, True/1 = CUDA-graph batches, 2 = graph batches whose kernels
-    are chained by programmatic dependent launch, 3 = one kernel resident on a thread-block cluster."""
+    are chained by programmatic dependent launch, 3 = one kernel resident on a thread-block cluster, 4 = one
+    cooperative kernel resident on all SMs."""
     g = nb.NBody(dev(pos), dev(vel), dev(m), eps, eta, dt_min=dt_min, dt_max=dt_max)
     nb.nb_set_loop_mode(g.ctx, int(graph))
     return g
@@ -41,7 +46,7 @@ def _same(sa, sb, mode, tol=1e-12):
     """Full states [n][21] = {m, t, dt, r, v, a, jerk, snap, crackle}: identical for the graph modes; for the
     resident loop m, t, dt identical and every 3-vector within tol of its own norm (crackle, a difference
     quotient of the evaluated values over h^3 that cancels heavily, within 1e-3)."""
-    if mode != 3:
+    if mode not in OWN_ORDER:
         return bool(np.array_equal(sa, sb))
     if not np.array_equal(sa[:, :3], sb[:, :3]):
         return False
@@ -53,7 +58,7 @@ def _same(sa, sb, mode, tol=1e-12):
     return True
 
 
-@pytest.mark.parametrize("mode", [1, 2, 3])
+@pytest.mark.parametrize("mode", [1, 2, 3, 4])
 @pytest.mark.parametrize("n,seed,eps,t_end", [(1024, 1, 1e-3, 0.25), (3000, 8, 1e-3, 0.0625), (77, 5, 1e-2, 0.5)])
 def test_graph_loop_is_bit_identical_to_call_sequence(nb, n, seed, eps, t_end, mode):
     if mode == 3 and n > 2048:
@@ -72,14 +77,14 @@ def test_graph_loop_is_bit_identical_to_call_sequence(nb, n, seed, eps, t_end, m
     # continue a second leg: the graph is replayed, not rebuilt, and the drivers still agree
     a.run_until(2 * t_end); b.run_until(2 * t_end)
     assert _same(_full(nb, a, n), _full(nb, b, n), mode)
-    if mode != 3:
+    if mode not in OWN_ORDER:
         assert np.array_equal(a.energy(), b.energy())
     else:
         assert abs(a.energy()[0] - b.energy()[0]) <= 1e-13 * abs(b.energy()[0])
     a.close(); b.close()
 
 
-@pytest.mark.parametrize("mode", [1, 3])
+@pytest.mark.parametrize("mode", [1, 3, 4])
 def test_graph_run_steps_counts_exactly(nb, mode):
     pos, vel, m = plummer(700, seed=21)
     a = _mk(nb, pos, vel, m, 1e-3, 0.45, 2.0 ** -25, 2.0 ** -4, graph=mode)
@@ -92,7 +97,7 @@ def test_graph_run_steps_counts_exactly(nb, mode):
     a.close(); b.close()
 
 
-@pytest.mark.parametrize("mode", [1, 3])
+@pytest.mark.parametrize("mode", [1, 3, 4])
 def test_graph_loop_then_single_calls(nb, mode):
     """Mixing drivers: a device-driven leg, then explicit calls, then a device-driven leg again."""
     pos, vel, m = plummer(500, seed=22)
@@ -108,7 +113,7 @@ def test_graph_loop_then_single_calls(nb, mode):
     a.close(); b.close()
 
 
-@pytest.mark.parametrize("mode", [1, 3])
+@pytest.mark.parametrize("mode", [1, 3, 4])
 def test_graph_loop_all_active_and_eps0(nb, mode):
     # shared step: every block has m = N (index-order evaluation, variant A at N >= 128)
     pos, vel, m = plummer(512, seed=3)
@@ -126,7 +131,7 @@ def test_graph_loop_all_active_and_eps0(nb, mode):
     a.close(); b.close()
 
 
-@pytest.mark.parametrize("mode", [1, 3])
+@pytest.mark.parametrize("mode", [1, 3, 4])
 def test_graph_loop_respects_tuning_knobs(nb, mode):
     """nb_set_tuning changes kernel arguments of the captured nodes: the graph is re-captured."""
     pos, vel, m = plummer(600, seed=23)
@@ -139,7 +144,7 @@ def test_graph_loop_respects_tuning_knobs(nb, mode):
     a.close(); b.close()
 
 
-@pytest.mark.parametrize("mode", [1, 3])
+@pytest.mark.parametrize("mode", [1, 3, 4])
 def test_graph_loop_matches_oracle_config1_quarter(nb, oracle, mode):
     pos, vel, m = plummer(1024, seed=1)
     g = _mk(nb, pos, vel, m, 1e-3, 0.45, 2.0 ** -25, 2.0 ** -4, graph=mode)
@@ -196,6 +201,46 @@ def test_resident_loop_limits_and_default(nb):
         assert sa_["n_pairs"] == sb_["n_pairs"] and list(sa_["hist"]) == list(sb_["hist"]) and sa_["t_now"] == sb_["t_now"]
         for g in (a, a2, b, d):
             g.close()
+
+
+def test_grid_resident_loop_limits_default_and_large_steps(nb):
+    """Mode 4 holds up to 704 particles per SM and is the default driver above 2048 particles while the system fits;
+    beyond that it refuses loudly.  At N = 20 011 (ragged: 136 particles per CTA on 148 SMs, the last CTAs partly
+    or wholly empty) the first block steps range from a handful of particles to more than 2048, so the run crosses
+    the hand-over of a large step to the call sequence and back several times.  Two runs are bit-identical."""
+    n = 20011
+    pos, vel, m = plummer(n, seed=27)
+    a = _mk(nb, pos, vel, m, 1e-4, 0.45, 2.0 ** -25, 2.0 ** -4, graph=4)
+    a2 = _mk(nb, pos, vel, m, 1e-4, 0.45, 2.0 ** -25, 2.0 ** -4, graph=4)
+    b = _mk(nb, pos, vel, m, 1e-4, 0.45, 2.0 ** -25, 2.0 ** -4, graph=False)
+    d = nb.NBody(dev(pos), dev(vel), dev(m), 1e-4, 0.45, dt_min=2.0 ** -25, dt_max=2.0 ** -4)   # default driver
+    k = a.run_until(2.0 ** -6)
+    assert k == b.run_until(2.0 ** -6) == a2.run_until(2.0 ** -6) == d.run_until(2.0 ** -6) and k > 100
+    sa = _full(nb, a, n)
+    assert _same(sa, _full(nb, b, n), 4)
+    assert np.array_equal(sa, _full(nb, a2, n))                # run-to-run bit-reproducible
+    assert np.array_equal(sa, _full(nb, d, n))                 # the default for this N is mode 4
+    sa_, sb_ = a.stats(), b.stats()
+    assert sa_["n_pairs"] == sb_["n_pairs"] and list(sa_["hist"]) == list(sb_["hist"]) and sa_["t_now"] == sb_["t_now"]
+    assert sb_["hist"][11:].sum() > 0 and sb_["hist"][:4].sum() > 0        # steps on both sides of the hand-over
+    # an exact step budget that ends inside a run of small steps, then inside the hand-over
+    for steps in (3, 40, 1):
+        a.run_steps(steps, log=False); b.run_steps(steps, log=False)
+        assert a.stats()["n_steps"] == b.stats()["n_steps"]
+    assert _same(_full(nb, a, n), _full(nb, b, n), 4)
+    # the predicted stream after a run is the prediction of the last step taken
+    pa, pb = [host(x) for x in a.pred()], [host(x) for x in b.pred()]
+    for x, y in zip(pa, pb):
+        assert np.abs(x - y).max() <= 1e-12 * np.abs(y).max()
+    for g in (a, a2, b, d):
+        g.close()
+    big = 704 * torch.cuda.get_device_properties(0).multi_processor_count + 1
+    pos, vel, m = plummer(big, seed=28)
+    g = nb.NBody(dev(pos), dev(vel), dev(m), 1e-3, 0.45, dt_min=2.0 ** -25, dt_max=2.0 ** -4)
+    with pytest.raises(nb.NBError) as e:
+        nb.nb_set_loop_mode(g.ctx, 4)
+    assert e.value.code == nb.nb.NB_EINVAL
+    g.close()
 
 
 def test_resident_loop_mixed_precision(nb):
