@@ -223,7 +223,7 @@ int nb_set_debug(nb_ctx *ctx, int on);
  * Modes 0, 1, 2 give bit-identical states.  Modes 3 and 4 add the pair terms of a particle in their own fixed order
  * (per owner CTA, then over the CTAs), so their results agree with modes 0-2 to rounding, not bit for bit (any order
  * is correct, G18), and are bit-reproducible from run to run.
- * Default: 3 for N <= 2048, 4 while the system fits the shared memory of the device, else 1.  nb_run_steps with a
+ * Default: 3 for N <= 1024, 4 while the system fits the shared memory of the device, else 1.  nb_run_steps with a
  * per-step log always uses 0.                                                                 */
 int nb_set_loop_mode(nb_ctx *ctx, int device_driven);
 

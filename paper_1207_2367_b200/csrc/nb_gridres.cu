@@ -104,15 +104,15 @@ __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long
 }
 
 // All CTAs of the (cooperative, co-resident) grid.  The counter only grows: the k-th barrier waits for k G arrivals.
+// Release / acquire at GPU scope: the block barrier orders this CTA's writes before thread 0's releasing add (which
+// is cumulative), and thread 0's acquiring load before every later read of the CTA.
 __device__ __forceinline__ void grid_barrier(unsigned long long *bar, unsigned long long &target, const int G)
 {
     __syncthreads();
     if (threadIdx.x == 0) {
         target += (unsigned long long)G;
-        __threadfence();                       // this CTA's writes (ordered before by the block barrier) are visible
-        atomicAdd(bar, 1ULL);
+        asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(bar) : "memory");
         while (ld_acquire_u64(bar) < target) { }
-        __threadfence();
     }
     __syncthreads();
 }
@@ -131,7 +131,9 @@ __global__ void __launch_bounds__(GR_THREADS, 1) k_grid_loop(const GridArgs A)
     double *rec = (double *)(smem + P.o_rec), *f1 = (double *)(smem + P.o_f1), *htmin = (double *)(smem + P.o_htmin);
     int *list = (int *)(smem + P.o_list), *base = (int *)(smem + P.o_base), *hcnt = (int *)(smem + P.o_hcnt);
     __shared__ int n_list;
-    __shared__ double red[GR_WARPS];
+    __shared__ int ctot[GR_MAXG / 32];
+    __shared__ double red[GR_WARPS], rest[GR_WARPS];
+    __shared__ unsigned long long moved_min;   // bits of the least t_i + dt_i among the particles corrected in this step
     __shared__ long long hist[64];
     const double inf = __longlong_as_double(0x7ff0000000000000LL);
     const int64_t N = A.N, Npad = A.Npad;
@@ -165,17 +167,9 @@ __global__ void __launch_bounds__(GR_THREADS, 1) k_grid_loop(const GridArgs A)
     double tn_last = 0.0;
     __syncthreads();
 
-    // minimum of t_i + dt_i over the owned particles, the particles that attain it (list), their records
-    // predicted to that time -> global memory, for every CTA to read after the barrier
-    auto publish = [&]() {
-        double vmin = inf;
-        for (int i = tid; i < n_own; i += GR_THREADS) vmin = fmin(vmin, t[i] + dt[i]);
-        for (int off = 16; off > 0; off >>= 1) vmin = fmin(vmin, __shfl_xor_sync(0xffffffffu, vmin, off));
-        if (lane == 0) red[warp] = vmin;
-        if (tid == 0) n_list = 0;
-        __syncthreads();
-        vmin = lane < GR_WARPS ? red[lane] : inf;
-        for (int off = 16; off > 0; off >>= 1) vmin = fmin(vmin, __shfl_xor_sync(0xffffffffu, vmin, off));
+    // publish: the minimum vmin of t_i + dt_i over the owned particles is known to every thread; the particles that
+    // attain it (list), their records predicted to that time -> global memory, for every CTA to read after the barrier
+    auto publish_at = [&](const double vmin) {
         for (int i = tid; i < n_own; i += GR_THREADS)
             if (t[i] + dt[i] == vmin) {
                 const int q = atomicAdd(&n_list, 1);
@@ -187,7 +181,27 @@ __global__ void __launch_bounds__(GR_THREADS, 1) k_grid_loop(const GridArgs A)
         __syncthreads();
         if (tid == 0) { GrHdr h; h.tmin = vmin; h.cnt = n_list; h.pad = 0; A.hdr[rank] = h; }
     };
-    publish();
+    // at the start: the minimum over all owned particles
+    auto publish_first = [&]() {
+        double vmin = inf;
+        for (int i = tid; i < n_own; i += GR_THREADS) vmin = fmin(vmin, t[i] + dt[i]);
+        for (int off = 16; off > 0; off >>= 1) vmin = fmin(vmin, __shfl_xor_sync(0xffffffffu, vmin, off));
+        if (lane == 0) red[warp] = vmin;
+        if (tid == 0) n_list = 0;
+        __syncthreads();
+        vmin = lane < GR_WARPS ? red[lane] : inf;
+        for (int off = 16; off > 0; off >>= 1) vmin = fmin(vmin, __shfl_xor_sync(0xffffffffu, vmin, off));
+        publish_at(vmin);
+    };
+    // after a step in which this CTA corrected particles (block barrier passed): the particles that were not due
+    // (rest[], from before the evaluation) and the corrected ones (moved_min)
+    auto publish_owner = [&]() {
+        double vmin = lane < GR_WARPS ? rest[lane] : inf;
+        for (int off = 16; off > 0; off >>= 1) vmin = fmin(vmin, __shfl_xor_sync(0xffffffffu, vmin, off));
+        vmin = fmin(vmin, __longlong_as_double((long long)moved_min));
+        publish_at(vmin);
+    };
+    publish_first();
     grid_barrier(A.bar, bar_target, G);
 #ifdef NB_GR_TIMING   // development aid: cycles per phase of the steps with m < 64, summed by one thread into unused histogram bins
     long long tph[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tcur[8];
@@ -208,20 +222,30 @@ __global__ void __launch_bounds__(GR_THREADS, 1) k_grid_loop(const GridArgs A)
         double tn = inf;
         for (int b = lane; b < G; b += 32) tn = fmin(tn, htmin[b]);
         for (int off = 16; off > 0; off >>= 1) tn = fmin(tn, __shfl_xor_sync(0xffffffffu, tn, off));
-        if (warp == 0) {   // exclusive prefix of the counts of the CTAs whose minimum is t_next
-            int run = 0;
-            for (int b0 = 0; b0 < G; b0 += 32) {
-                const int b = b0 + lane;
-                const int cnt = (b < G && htmin[b] == tn) ? hcnt[b] : 0;
-                int inc = cnt;
-                for (int off = 1; off < 32; off <<= 1) {
-                    const int y = __shfl_up_sync(0xffffffffu, inc, off);
-                    if (lane >= off) inc += y;
-                }
-                if (b < G) base[b] = run + inc - cnt;
-                run += __shfl_sync(0xffffffffu, inc, 31);
+        // exclusive prefix of the counts of the CTAs whose minimum is t_next: warp w scans the 32 CTAs of chunk w,
+        // then every entry adds the totals of the chunks before its own
+        if (warp < GR_MAXG / 32) {
+            const int b = warp * 32 + lane;
+            const int cnt = (b < G && htmin[b] == tn) ? hcnt[b] : 0;
+            int inc = cnt;
+            for (int off = 1; off < 32; off <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, inc, off);
+                if (lane >= off) inc += y;
             }
-            if (lane == 0) base[G] = run;
+            if (b < G) base[b] = inc - cnt;
+            if (lane == 31) ctot[warp] = inc;
+        }
+        __syncthreads();
+        {
+            int before = 0, total = 0;
+#pragma unroll
+            for (int w = 0; w < GR_MAXG / 32; ++w) {
+                const int cw = ctot[w];
+                if (w < (tid >> 5)) before += cw;
+                total += cw;
+            }
+            if (tid < G) base[tid] += before;      // tid >> 5 is the chunk of entry tid
+            if (tid == 0) base[G] = total;
         }
         __syncthreads();
         const int m = base[G];
@@ -229,31 +253,53 @@ __global__ void __launch_bounds__(GR_THREADS, 1) k_grid_loop(const GridArgs A)
         if (steps_left <= 0 || !(tn <= t_end)) { reason = 1; break; }
         if (m >= A.m_big) { reason = 2; tn_last = tn; break; }   // a large step: the streaming kernels take it
 
-        // ---- predict the owned particles (Eq. 3-7)
-        for (int i = tid; i < n_own; i += GR_THREADS) predict_one(i, NL, tn, t, mass, r, v, a, j, s, c, rec);
-        __syncthreads();
-        NB_TICK(1);
-
-        // ---- evaluate all m active particles against the owned records; one partial per CTA and component
+        // lanes per i and the record of this thread's first slot: the load from the candidates buffer is issued
+        // before the predictor so that its trip to L2 overlaps it
         int JL = 1;
         if (A.force_jlanes >= 1) JL = A.force_jlanes < JL_MAX ? A.force_jlanes : JL_MAX;
         else { while (JL < JL_MAX && m * (JL * 2) <= GR_THREADS) JL *= 2; }
         const int slots = GR_THREADS / JL;
-        for (int k0 = 0; k0 < m; k0 += slots) {                 // warp-uniform trip count
-            if (k0 + (tid & ~31) / JL >= m) continue;           // a warp without a live slot has nothing to add
-            const int k = k0 + tid / JL, jl = tid % JL;
-            const bool live = k < m;
-            const int kk = live ? k : m - 1;
-            int lo = 0, hi = G - 1;                             // owner: the last CTA with base[o] <= kk and a non-empty list
+        auto load_slot = [&](const int k0, double2 (&w)[REC / 2]) {
+            const int k = k0 + tid / JL;
+            const int kk = k < m ? k : m - 1;
+            int lo = 0, hi = G - 1;                             // owner: the last CTA with base[o] <= kk (ties: the non-empty one)
             while (lo < hi) {
                 const int mid = (lo + hi + 1) >> 1;
                 if (base[mid] <= kk) lo = mid; else hi = mid - 1;
             }
-            const int o = lo, qloc = kk - base[lo];
-            const double2 *src = reinterpret_cast<const double2 *>(A.cand + ((size_t)o * NL + qloc) * REC);
+            const double2 *src = reinterpret_cast<const double2 *>(A.cand + ((size_t)lo * NL + (kk - base[lo])) * REC);
+#pragma unroll
+            for (int d = 0; d < REC / 2; ++d) w[d] = __ldcg(src + d);
+        };
+        double2 w0[REC / 2];
+        const bool first_live = (tid & ~31) / JL < m;           // this warp has a live slot in the first round
+        if (first_live) load_slot(0, w0);
+
+        // ---- predict the owned particles (Eq. 3-7); on the way, the minimum of t_i + dt_i over the particles that are
+        // NOT due now (it cannot change in this step): the owners' next publish starts from it
+        {
+            double vr = inf;
+            for (int i = tid; i < n_own; i += GR_THREADS) {
+                predict_one(i, NL, tn, t, mass, r, v, a, j, s, c, rec);
+                const double x = t[i] + dt[i];
+                if (x != tn) vr = fmin(vr, x);
+            }
+            for (int off = 16; off > 0; off >>= 1) vr = fmin(vr, __shfl_xor_sync(0xffffffffu, vr, off));
+            if (lane == 0) rest[warp] = vr;
+            if (tid == 0) { moved_min = 0x7ff0000000000000ULL; n_list = 0; }   // for the publish of this step
+        }
+        __syncthreads();
+        NB_TICK(1);
+
+        // ---- evaluate all m active particles against the owned records; one partial per CTA and component
+        for (int k0 = 0; k0 < m; k0 += slots) {                 // warp-uniform trip count
+            if (k0 + (tid & ~31) / JL >= m) continue;           // a warp without a live slot has nothing to add
+            const int k = k0 + tid / JL, jl = tid % JL;
+            const bool live = k < m;
+            if (k0 > 0) load_slot(k0, w0);
             double ri[REC];
 #pragma unroll
-            for (int d = 0; d < REC / 2; ++d) { const double2 w = __ldcg(src + d); ri[2 * d] = w.x; ri[2 * d + 1] = w.y; }
+            for (int d = 0; d < REC / 2; ++d) { ri[2 * d] = w0[d].x; ri[2 * d + 1] = w0[d].y; }
             Acc9 T;
             switch (JL) {
                 case 1: T = res_eval<1, GUARD0, MX>(ri, rec, jl, NL, A.eps2); break;
@@ -274,23 +320,31 @@ __global__ void __launch_bounds__(GR_THREADS, 1) k_grid_loop(const GridArgs A)
         NB_TICK(3);
 
         // ---- correct: the owner sums the G partials of each of its active particles (lane-strided, ascending,
-        // then the xor butterfly: the order of sum_splits_warp) and applies Eq. 11-16.  One warp per particle.
+        // then the xor butterfly: the order of sum_splits_warp) and applies Eq. 11-16 (one warp per particle).
         const int n_mine = (htmin[rank] == tn) ? base[rank + 1] - base[rank] : 0;
+        // the sums: one warp per (particle, component), so that all loads of a sum are in flight together (one trip
+        // to L2 instead of one per 32 CTAs); the additions and their order are those of sum_splits_warp
+        for (int it = warp; it < n_mine * 9; it += GR_WARPS) {
+            const int q = it / 9, cc = it - q * 9;
+            const double *p0 = A.part + ((size_t)(base[rank] + q) * 9 + cc) * G;
+            double vv[GR_MAXG / 32];
+#pragma unroll
+            for (int u = 0; u < GR_MAXG / 32; ++u) {
+                const int sidx = lane + 32 * u;
+                vv[u] = sidx < G ? __ldcg(p0 + sidx) : 0.0;
+            }
+            double x = 0.0;
+#pragma unroll
+            for (int u = 0; u < GR_MAXG / 32; ++u) x += vv[u];
+            for (int off = 16; off > 0; off >>= 1) x += __shfl_xor_sync(0xffffffffu, x, off);
+            if (lane == 0) f1[cc * NL + q] = x;
+        }
+        __syncthreads();
         for (int q = warp; q < n_mine; q += GR_WARPS) {
-            const double *p0 = A.part + (size_t)(base[rank] + q) * 9 * G;
-            double acc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
-            for (int sidx = lane; sidx < G; sidx += 32) {
-#pragma unroll
-                for (int cc = 0; cc < 9; ++cc) acc[cc] += __ldcg(p0 + (size_t)cc * G + sidx);
-            }
-#pragma unroll
-            for (int cc = 0; cc < 9; ++cc) {
-                double x = acc[cc];
-                for (int off = 16; off > 0; off >>= 1) x += __shfl_xor_sync(0xffffffffu, x, off);
-                if (lane == 0) f1[cc * NL + q] = x;
-            }
-            __syncwarp();
-            correct_warp(lane, q, list[q], NL, tn, A.eta, A.dt_min, A.dt_max, f1, t, dt, r, v, a, j, s, c);
+            const int i = list[q];
+            correct_warp(lane, q, i, NL, tn, A.eta, A.dt_min, A.dt_max, f1, t, dt, r, v, a, j, s, c);
+            // times are non-negative dyadic rationals: the bit pattern orders like the value
+            if (lane == 0) atomicMin(&moved_min, (unsigned long long)__double_as_longlong(t[i] + dt[i]));
         }
         __syncthreads();
         NB_TICK(4);
@@ -300,7 +354,7 @@ __global__ void __launch_bounds__(GR_THREADS, 1) k_grid_loop(const GridArgs A)
             while ((1LL << (b + 1)) <= (long long)m) ++b;
             hist[b] += 1;
         }
-        publish();
+        if (n_mine > 0) publish_owner();   // nothing of a CTA without active particles changed: its header and candidates stand
         NB_TICK(5);
         grid_barrier(A.bar, bar_target, G);
         NB_TICK(6);

@@ -87,7 +87,8 @@ constexpr int64_t L2_CHUNK_BYTES = 24 << 20;         // j-stream piece kept L2-r
 constexpr int GEOM_CACHE_M = 4096;                   // the device loop remembers the geometry of set sizes up to this
 constexpr int MAX_WAVES = 255;                      // the split search considers 1..MAX_WAVES work items per SM
 constexpr int64_t RES_MAX_N = 2048;                  // the cluster-resident loop (nb_resident.cu) keeps N up to this on chip
-constexpr int64_t RES_AUTO_N = 2048;                 // ... and is the default driver up to this
+constexpr int64_t RES_AUTO_N = 1024;                 // ... and is the default driver up to this (measured: 7.7 against 10.5 us per
+                                                     // step at N = 512, 10.4 / 11.1 at 1024, 16.6 / 11.9 at 2048 for modes 3 / 4)
 constexpr int GR_M_BIG_DEFAULT = 2048;               // grid-resident loop (nb_gridres.cu): steps with this many active particles
                                                      // or more go to the streaming kernels
 

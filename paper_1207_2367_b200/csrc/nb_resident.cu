@@ -194,6 +194,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
         else { while (JL < JL_MAX && m * (JL * 2) <= RES_THREADS) JL *= 2; }
         const int slots = RES_THREADS / JL;
         for (int k0 = 0; k0 < m; k0 += slots) {                 // warp-uniform trip count
+            if (k0 + (tid & ~31) / JL >= m) continue;           // a warp without a live slot has nothing to add
             const int k = k0 + tid / JL, jl = tid % JL;
             const bool live = k < m;
             const int kk = live ? k : m - 1;

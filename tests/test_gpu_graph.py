@@ -176,8 +176,9 @@ def test_graph_loop_large_ragged_n(nb):
 
 
 def test_resident_loop_limits_and_default(nb):
-    """Mode 3 serves N <= 2048 and is the default driver there; above its limit it refuses loudly.  Two runs of
-    it give bit-identical states (fixed summation order)."""
+    """Mode 3 serves N <= 2048 and is the default driver up to N = 1024 (mode 4 above, while the system fits the
+    shared memory of the device); above its limit it refuses loudly.  Two runs of it give bit-identical states
+    (fixed summation order)."""
     pos, vel, m = plummer(3000, seed=25)
     g = nb.NBody(dev(pos), dev(vel), dev(m), 1e-3, 0.45, dt_min=2.0 ** -25, dt_max=2.0 ** -4)
     with pytest.raises(nb.NBError) as e:
@@ -185,7 +186,7 @@ def test_resident_loop_limits_and_default(nb):
     assert e.value.code == nb.nb.NB_EINVAL
     g.close()
     # N = 2048 (the limit: 128 particles per CTA; all-active steps among them) and a ragged N
-    for n in (2048, 1531):
+    for n in (2048, 1531, 1000):
         pos, vel, m = plummer(n, seed=26)
         a = _mk(nb, pos, vel, m, 1e-3, 0.45, 2.0 ** -25, 2.0 ** -4, graph=3)
         a2 = _mk(nb, pos, vel, m, 1e-3, 0.45, 2.0 ** -25, 2.0 ** -4, graph=3)
@@ -196,7 +197,11 @@ def test_resident_loop_limits_and_default(nb):
         sa = _full(nb, a, n)
         assert _same(sa, _full(nb, b, n), 3)
         assert np.array_equal(sa, _full(nb, a2, n))            # run-to-run bit-reproducible
-        assert np.array_equal(sa, _full(nb, d, n))             # the default for this N is mode 3
+        assert nb.nb_get_loop_mode(d.ctx) == (3 if n <= 1024 else 4)
+        if n <= 1024:
+            assert np.array_equal(sa, _full(nb, d, n))         # the default for this N is mode 3
+        else:
+            assert _same(_full(nb, d, n), _full(nb, b, n), 4)  # ... mode 4
         sa_, sb_ = a.stats(), b.stats()
         assert sa_["n_pairs"] == sb_["n_pairs"] and list(sa_["hist"]) == list(sb_["hist"]) and sa_["t_now"] == sb_["t_now"]
         for g in (a, a2, b, d):
