@@ -248,14 +248,29 @@ def test_grid_resident_loop_limits_default_and_large_steps(nb):
     g.close()
 
 
-def test_resident_loop_mixed_precision(nb):
-    """Mixed SP/DP pair arithmetic (reading G27) inside the resident loop: float rounding in another order moves
+def test_grid_resident_loop_every_step_large(nb):
+    """A shared time step (dt_min = dt_max) at N = 4096 >= the hand-over threshold: EVERY block step has m = N and goes
+    to the call sequence with the all-particles list; the grid-resident kernel only selects.  Bit-identical to mode 0."""
+    n = 4096
+    pos, vel, m = plummer(n, seed=29)
+    a = _mk(nb, pos, vel, m, 1e-2, 0.45, 2.0 ** -8, 2.0 ** -8, graph=4)
+    b = _mk(nb, pos, vel, m, 1e-2, 0.45, 2.0 ** -8, 2.0 ** -8, graph=False)
+    assert a.run_until(2.0 ** -5) == 8 and b.run_until(2.0 ** -5) == 8
+    assert np.array_equal(_full(nb, a, n), _full(nb, b, n))
+    a.run_steps(3, log=False); b.run_steps(3, log=False)
+    assert np.array_equal(_full(nb, a, n), _full(nb, b, n)) and a.stats()["n_pairs"] == b.stats()["n_pairs"]
+    a.close(); b.close()
+
+
+@pytest.mark.parametrize("mode", [3, 4])
+def test_resident_loop_mixed_precision(nb, mode):
+    """Mixed SP/DP pair arithmetic (reading G27) inside the resident loops: float rounding in another order moves
     individual time-step decisions, so only the integrated quantities are compared with the call sequence."""
     # config 1's system with a wide floor on the step (2^-12): single-precision forces can drive the 6th-order
     # step rule of a particle in a close encounter down to dt_min (DESIGN.md section 13); that is a property of the
     # mode, not of the driver, and would only make this comparison long
     pos, vel, m = plummer(1024, seed=1)
-    a = _mk(nb, pos, vel, m, 1e-3, 0.45, 2.0 ** -12, 2.0 ** -4, graph=3)
+    a = _mk(nb, pos, vel, m, 1e-3, 0.45, 2.0 ** -12, 2.0 ** -4, graph=mode)
     b = _mk(nb, pos, vel, m, 1e-3, 0.45, 2.0 ** -12, 2.0 ** -4, graph=False)
     nb.nb_set_precision(a.ctx, 1); nb.nb_set_precision(b.ctx, 1)
     a.startup(); b.startup()
