@@ -221,6 +221,14 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
                 dst[6] = T.sx; dst[7] = T.sy; dst[8] = T.sz;
             }
         }
+#ifdef NB_RES_TIMING
+        {   // phase-2 cycles by floor(log2 m) -> bins 48 + b (development aid)
+            const long long now_ = clock64();
+            int b_ = 0;
+            while ((1LL << (b_ + 1)) <= (long long)m) ++b_;
+            if (rank == 0 && tid == 0 && b_ < 15) hist[48 + b_] += now_ - tq;
+        }
+#endif
         NB_TICK(3);
         cluster.sync();
         NB_TICK(4);
