@@ -255,12 +255,13 @@ __global__ void __launch_bounds__(GR_THREADS, 1) k_grid_loop(const GridArgs A)
 
         // lanes per i and the record of this thread's first slot: the load from the candidates buffer is issued
         // before the predictor so that its trip to L2 overlaps it
-        int JL = 1;
-        if (A.force_jlanes >= 1) JL = A.force_jlanes < JL_MAX ? A.force_jlanes : JL_MAX;
-        else { while (JL < JL_MAX && m * (JL * 2) <= GR_THREADS) JL *= 2; }
-        const int slots = GR_THREADS / JL;
+        int lj = 0;                                             // JL = 2^lj lanes per i: shifts, not divisions, below
+        if (A.force_jlanes >= 1) { const int want = A.force_jlanes < JL_MAX ? A.force_jlanes : JL_MAX; while ((2 << lj) <= want) ++lj; }
+        else { while ((2 << lj) <= JL_MAX && (m << (lj + 1)) <= GR_THREADS) ++lj; }
+        const int JL = 1 << lj;
+        const int slots = GR_THREADS >> lj;
         auto load_slot = [&](const int k0, double2 (&w)[REC / 2]) {
-            const int k = k0 + tid / JL;
+            const int k = k0 + (tid >> lj);
             const int kk = k < m ? k : m - 1;
             int lo = 0, hi = G - 1;                             // owner: the last CTA with base[o] <= kk (ties: the non-empty one)
             while (lo < hi) {
@@ -272,7 +273,7 @@ __global__ void __launch_bounds__(GR_THREADS, 1) k_grid_loop(const GridArgs A)
             for (int d = 0; d < REC / 2; ++d) w[d] = __ldcg(src + d);
         };
         double2 w0[REC / 2];
-        const bool first_live = (tid & ~31) / JL < m;           // this warp has a live slot in the first round
+        const bool first_live = ((tid & ~31) >> lj) < m;           // this warp has a live slot in the first round
         if (first_live) load_slot(0, w0);
 
         // ---- predict the owned particles (Eq. 3-7); on the way, the minimum of t_i + dt_i over the particles that are
@@ -293,8 +294,8 @@ __global__ void __launch_bounds__(GR_THREADS, 1) k_grid_loop(const GridArgs A)
 
         // ---- evaluate all m active particles against the owned records; one partial per CTA and component
         for (int k0 = 0; k0 < m; k0 += slots) {                 // warp-uniform trip count
-            if (k0 + (tid & ~31) / JL >= m) continue;           // a warp without a live slot has nothing to add
-            const int k = k0 + tid / JL, jl = tid % JL;
+            if (k0 + ((tid & ~31) >> lj) >= m) continue;           // a warp without a live slot has nothing to add
+            const int k = k0 + (tid >> lj), jl = tid & (JL - 1);
             const bool live = k < m;
             if (k0 > 0) load_slot(k0, w0);
             double ri[REC];

@@ -189,13 +189,14 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
 #pragma unroll
         for (int o = 0; o < RES_MAXC; ++o) base[o + 1] = base[o] + (o < C ? cnt[o] : 0);
         const int m = base[RES_MAXC];
-        int JL = 1;
-        if (force_jlanes >= 1) JL = force_jlanes < JL_MAX ? force_jlanes : JL_MAX;
-        else { while (JL < JL_MAX && m * (JL * 2) <= RES_THREADS) JL *= 2; }
-        const int slots = RES_THREADS / JL;
+        int lj = 0;                                             // JL = 2^lj lanes per i: shifts, not divisions, below
+        if (force_jlanes >= 1) { const int want = force_jlanes < JL_MAX ? force_jlanes : JL_MAX; while ((2 << lj) <= want) ++lj; }
+        else { while ((2 << lj) <= JL_MAX && (m << (lj + 1)) <= RES_THREADS) ++lj; }
+        const int JL = 1 << lj;
+        const int slots = RES_THREADS >> lj;
         for (int k0 = 0; k0 < m; k0 += slots) {                 // warp-uniform trip count
-            if (k0 + (tid & ~31) / JL >= m) continue;           // a warp without a live slot has nothing to add
-            const int k = k0 + tid / JL, jl = tid % JL;
+            if (k0 + ((tid & ~31) >> lj) >= m) continue;           // a warp without a live slot has nothing to add
+            const int k = k0 + (tid >> lj), jl = tid & (JL - 1);
             const bool live = k < m;
             const int kk = live ? k : m - 1;
             int o = 0, bo = 0;                                  // owner CTA of slot kk and the first slot it owns
