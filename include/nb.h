@@ -171,7 +171,9 @@ int nb_get_stats(nb_ctx *ctx, double out[4], int64_t hist[64]);
 
 /* Tuning knobs of the evaluation kernel, for the split-j on/off experiment (PAPER.md:256,
  * Fig. 8): split = 0 chooses the number of j-splits automatically (default), split >= 1
- * forces it.  jlanes = 0 automatic, else lanes of a warp that share one i (1, 2, 4 .. 32).  */
+ * forces it.  jlanes = 0 automatic, else lanes of a warp that share one i (1, 2, 4 .. 32).
+ * The resident loops (nb_set_loop_mode 3, 4) split the j-range by construction (one piece per CTA) and honour
+ * jlanes only.                                                                               */
 int nb_set_tuning(nb_ctx *ctx, int split, int jlanes);
 
 /* j-sharding across GPUs (the paper's decomposition; Table 1 row 7): every
