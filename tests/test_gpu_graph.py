@@ -248,6 +248,23 @@ def test_grid_resident_loop_limits_default_and_large_steps(nb):
     g.close()
 
 
+def test_grid_resident_loop_matches_oracle(nb, oracle):
+    """The default driver above N = 1024 against the oracle's Hermite loop directly (N = 4000, ragged over 148 CTAs):
+    same number of block steps, identical t_i and dt_i (every time-step decision), positions within 1e-9."""
+    n = 4000
+    pos, vel, m = plummer(n, seed=30)
+    g = nb.NBody(dev(pos), dev(vel), dev(m), 1e-3, 0.45, dt_min=2.0 ** -25, dt_max=2.0 ** -4)
+    assert nb.nb_get_loop_mode(g.ctx) == 4
+    k = g.run_until(2.0 ** -6)
+    it = oracle.Integrator(pos, vel, m, eps=1e-3, eta=0.45, dt_min=2.0 ** -25, dt_max=2.0 ** -4)
+    assert it.run_until(2.0 ** -6)[0] == k and k > 50
+    r, v, t, dt = [host(x) for x in g.state()]
+    assert np.array_equal(t, it.t) and np.array_equal(dt, it.dt)
+    assert (np.linalg.norm(r - it.pos, axis=1) / np.linalg.norm(it.pos, axis=1)).max() < 1e-9
+    assert (np.linalg.norm(v - it.vel, axis=1) / np.linalg.norm(it.vel, axis=1)).max() < 1e-8
+    g.close()
+
+
 def test_grid_resident_loop_every_step_large(nb):
     """A shared time step (dt_min = dt_max) at N = 4096 >= the hand-over threshold: EVERY block step has m = N and goes
     to the call sequence with the all-particles list; the grid-resident kernel only selects.  Bit-identical to mode 0."""
