@@ -46,7 +46,7 @@ constexpr int RES_PUSH = 16;        // each owner pushes the records of its firs
 //   state  : t, dt, mass [NL]; r, v, a, jerk, snap, crackle [3][NL]      21 NL
 //   rec    : predicted records [NL][REC]                                   10 NL
 //   f1     : reduced (a, jerk, snap) of the owned active particles [9][NL]  9 NL
-//   part   : partials [NL][C][9] written by every CTA of the cluster       9 C NL
+//   part   : partials [C][9][NL] (writer CTA, component, slot), written by every CTA of the cluster   9 C NL
 //   irec   : records of the first RES_PUSH due particles of every CTA [16][RES_PUSH][REC], pushed by their owners
 //            (a small active set is then evaluated without a read from remote shared memory)
 //   tmin   : min(t_i + dt_i) of every CTA [16];  list: int32 local indices of the owned due particles [NL];
@@ -194,11 +194,15 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
         else { while ((2 << lj) <= JL_MAX && (m << (lj + 1)) <= RES_THREADS) ++lj; }
         const int JL = 1 << lj;
         const int slots = RES_THREADS >> lj;
+        const int rot = (int)(((long long)rank * m) / C);
         for (int k0 = 0; k0 < m; k0 += slots) {                 // warp-uniform trip count
             if (k0 + ((tid & ~31) >> lj) >= m) continue;           // a warp without a live slot has nothing to add
             const int k = k0 + (tid >> lj), jl = tid & (JL - 1);
             const bool live = k < m;
-            const int kk = live ? k : m - 1;
+            // every CTA walks the slots in its own rotation, so that at any moment the 16 CTAs read the records of, and
+            // store partial sums to, different owners instead of all pressing on the same few
+            int kk = (live ? k : m - 1) + rot;
+            if (kk >= m) kk -= m;
             int o = 0, bo = 0;                                  // owner CTA of slot kk and the first slot it owns
 #pragma unroll
             for (int q = 1; q < RES_MAXC; ++q)
@@ -207,6 +211,13 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
             const double *ri;
             if (qloc < RES_PUSH) ri = irec + ((size_t)o * RES_PUSH + qloc) * REC;     // pushed by its owner in phase 1
             else ri = cluster.map_shared_rank(rec, o) + (size_t)cluster.map_shared_rank(list, o)[qloc] * REC;
+            double rl[REC];                                     // the i-record in five 16-byte loads (local or remote)
+#pragma unroll
+            for (int d = 0; d < REC / 2; ++d) {
+                const double2 w = reinterpret_cast<const double2 *>(ri)[d];
+                rl[2 * d] = w.x; rl[2 * d + 1] = w.y;
+            }
+            ri = rl;
             Acc9 T;
             switch (JL) {
                 case 1: T = res_eval<1, GUARD0, MX>(ri, rec, jl, NL, eps2); break;
@@ -217,9 +228,11 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
                 default: T = res_eval<32, GUARD0, MX>(ri, rec, jl, NL, eps2); break;
             }
             if (live && jl == 0) {
-                double *dst = cluster.map_shared_rank(part, o) + ((size_t)qloc * C + rank) * 9;
-                dst[0] = T.ax; dst[1] = T.ay; dst[2] = T.az; dst[3] = T.jx; dst[4] = T.jy; dst[5] = T.jz;
-                dst[6] = T.sx; dst[7] = T.sy; dst[8] = T.sz;
+                // part[writer][component][slot]: the lanes of a warp hold consecutive slots of (mostly) one owner, so each
+                // of the nine remote stores of a warp is one contiguous row in the owner's shared memory
+                double *dst = cluster.map_shared_rank(part, o) + (size_t)rank * 9 * NL + qloc;
+                dst[0 * NL] = T.ax; dst[1 * NL] = T.ay; dst[2 * NL] = T.az; dst[3 * NL] = T.jx; dst[4 * NL] = T.jy;
+                dst[5 * NL] = T.jz; dst[6 * NL] = T.sx; dst[7 * NL] = T.sy; dst[8 * NL] = T.sz;
             }
         }
 #ifdef NB_RES_TIMING
@@ -237,14 +250,29 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
         // ---- phase 3: the owner sums the C partials of each of its active particles in rank order and
         // corrects it (Eq. 11-16).  One warp per particle: lanes 0..8 take one component each.
         const int n_mine = cnt[rank];
-        for (int q = warp; q < n_mine; q += RES_WARPS) {
-            if (lane < 9) {
-                double acc = 0.0;
-                for (int o = 0; o < C; ++o) acc += part[((size_t)q * C + o) * 9 + lane];
-                f1[lane * NL + q] = acc;
+        if (n_mine <= RES_WARPS) {
+            for (int q = warp; q < n_mine; q += RES_WARPS) {
+                if (lane < 9) {
+                    double acc = 0.0;
+                    for (int o = 0; o < C; ++o) acc += part[((size_t)o * 9 + lane) * NL + q];
+                    f1[lane * NL + q] = acc;
+                }
+                __syncwarp();
+                correct_warp(lane, q, list[q], NL, tn, eta, dt_min, dt_max, f1, t, dt, r, v, a, j, s, c);
             }
-            __syncwarp();
-            correct_warp(lane, q, list[q], NL, tn, eta, dt_min, dt_max, f1, t, dt, r, v, a, j, s, c);
+        } else {
+            // many active particles per CTA (a large step): one thread per (particle, component) for the sums, then one
+            // thread per particle for the corrector (correct_one: the expressions and rounding order of correct_warp);
+            // a warp taking several particles in turn would run their dependent chains one after the other
+            for (int e = tid; e < n_mine * 9; e += RES_THREADS) {
+                const int cc = e / n_mine, q = e - cc * n_mine;     // consecutive threads: consecutive slots
+                double acc = 0.0;
+                for (int o = 0; o < C; ++o) acc += part[((size_t)o * 9 + cc) * NL + q];
+                f1[cc * NL + q] = acc;
+            }
+            __syncthreads();
+            for (int q = tid; q < n_mine; q += RES_THREADS)
+                correct_one(q, list[q], NL, tn, eta, dt_min, dt_max, f1, t, dt, r, v, a, j, s, c);
         }
         __syncthreads();
         steps_left -= 1; n_steps += 1; n_pairs += (double)m * (double)N; t_now = tn;
