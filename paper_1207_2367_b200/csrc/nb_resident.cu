@@ -95,6 +95,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
     cg::cluster_group cluster = cg::this_cluster();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
+    const int lgC = 31 - __clz(C);                                  // the cluster has 8 or 16 CTAs
     const ResPlan P = res_plan(N, C);
     const int NL = P.NL;
     double *t = (double *)(smem + P.o_t), *dt = (double *)(smem + P.o_dt), *mass = (double *)(smem + P.o_m);
@@ -184,17 +185,20 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
         NB_TICK(2);
 
         // ---- phase 2: all m active particles against the owned records; partials to the owners
-        int base[RES_MAXC + 1];
-        base[0] = 0;
+        // inclusive prefix of the owners' list lengths, one per lane (lanes >= C hold the total): a warp scan
+        int inc = lane < C ? cnt[lane] : 0;
 #pragma unroll
-        for (int o = 0; o < RES_MAXC; ++o) base[o + 1] = base[o] + (o < C ? cnt[o] : 0);
-        const int m = base[RES_MAXC];
+        for (int off = 1; off < RES_MAXC; off <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, inc, off);
+            if (lane >= off) inc += y;
+        }
+        const int m = __shfl_sync(0xffffffffu, inc, RES_MAXC - 1);
         int lj = 0;                                             // JL = 2^lj lanes per i: shifts, not divisions, below
         if (force_jlanes >= 1) { const int want = force_jlanes < JL_MAX ? force_jlanes : JL_MAX; while ((2 << lj) <= want) ++lj; }
         else { while ((2 << lj) <= JL_MAX && (m << (lj + 1)) <= RES_THREADS) ++lj; }
         const int JL = 1 << lj;
         const int slots = RES_THREADS >> lj;
-        const int rot = (int)(((long long)rank * m) / C);
+        const int rot = (rank * m) >> lgC;                      // m <= 2048, rank < 16
         for (int k0 = 0; k0 < m; k0 += slots) {                 // warp-uniform trip count
             if (k0 + ((tid & ~31) >> lj) >= m) continue;           // a warp without a live slot has nothing to add
             const int k = k0 + (tid >> lj), jl = tid & (JL - 1);
@@ -203,10 +207,19 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
             // store partial sums to, different owners instead of all pressing on the same few
             int kk = (live ? k : m - 1) + rot;
             if (kk >= m) kk -= m;
-            int o = 0, bo = 0;                                  // owner CTA of slot kk and the first slot it owns
+            int o, bo;                                          // owner CTA of slot kk and the first slot it owns:
+            if (lj == 5) {                                      // one slot per warp (m <= 16): every lane asks the same
+                o = __popc(__ballot_sync(0xffffffffu, lane < RES_MAXC && inc <= kk));   // owners wholly before slot kk
+                bo = __shfl_sync(0xffffffffu, inc, o > 0 ? o - 1 : 0);
+                if (o == 0) bo = 0;
+            } else {
+                o = 0; bo = 0;
 #pragma unroll
-            for (int q = 1; q < RES_MAXC; ++q)
-                if (q < C && kk >= base[q]) { o = q; bo = base[q]; }
+                for (int q = 1; q < RES_MAXC; ++q) {
+                    const int bq = __shfl_sync(0xffffffffu, inc, q - 1);
+                    if (q < C && kk >= bq) { o = q; bo = bq; }
+                }
+            }
             const int qloc = kk - bo;                           // slot in the owner's list
             const double *ri;
             if (qloc < RES_PUSH) ri = irec + ((size_t)o * RES_PUSH + qloc) * REC;     // pushed by its owner in phase 1

@@ -34,9 +34,14 @@ __device__ __forceinline__ Acc9 res_eval(const double *ri, const double *rec, co
             T.sx += (double)A.sx; T.sy += (double)A.sy; T.sz += (double)A.sz;
         }
     } else {
+        if (per == 2) {   // the usual case of a small system (64 records per CTA, 32 lanes per i): the two pairs overlap
+            pair_body<GUARD0, true>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q, eps2, T);
+            pair_body<GUARD0, true>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + (size_t)(JL * REC), eps2, T);
+        } else {
 #pragma unroll 8
-        for (int jj = 0; jj < per; ++jj)
-            pair_body<GUARD0, true>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + (size_t)jj * (JL * REC), eps2, T);
+            for (int jj = 0; jj < per; ++jj)
+                pair_body<GUARD0, true>(xi, yi, zi, vxi, vyi, vzi, axi, ayi, azi, q + (size_t)jj * (JL * REC), eps2, T);
+        }
     }
     if (MX == 0) {  // the FP64 pair body accumulates 3 sqrt(3) times the sums (pair_body)
         T.ax *= PAIR_SCALE; T.ay *= PAIR_SCALE; T.az *= PAIR_SCALE;
@@ -69,7 +74,9 @@ __device__ __forceinline__ void correct_warp(const int lane, const int k, const 
     if (lane < 3) {
         const int d = lane;
         const double h2 = h * h, h3 = h2 * h;
-        const double ih = 1.0 / h;  // exact: h is a power of two
+        // 1 / h for h = 2^k, exactly, from the exponent field (an IEEE division is a few hundred cycles of dependent
+        // instructions on the path every owner walks between two barriers): bits(2^-k) = (2046 << 52) - bits(2^k)
+        const double ih = __longlong_as_double((2046LL << 52) - __double_as_longlong(h));
         const double ih3 = ih * ih * ih, ih4 = ih3 * ih, ih5 = ih4 * ih;
         const int q = d * NL + i;
         const double r0 = r[q], v0 = v[q], a0 = a[q], j0 = j[q], s0 = s[q];
