@@ -105,7 +105,6 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
     double *tmin = (double *)(smem + P.o_tmin), *irec = (double *)(smem + P.o_irec);
     int *list = (int *)(smem + P.o_list), *cnt = (int *)(smem + P.o_cnt);
     __shared__ int n_list;
-    __shared__ double red[RES_WARPS];
     __shared__ long long hist[64];
     const double inf = __longlong_as_double(0x7ff0000000000000LL);
     const int64_t first = (int64_t)rank * NL;                       // first owned particle
@@ -135,16 +134,15 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
     __syncthreads();
 
     // minimum of t_i + dt_i over the owned particles -> tmin[rank] of every CTA
+    // (one warp does it: a CTA owns at most RES_NL_MAX = 256 particles, eight per lane; the callers have just passed a
+    // block barrier, so the corrected times are visible; no barrier inside)
     auto publish_min = [&]() {
-        double vmin = inf;
-        for (int i = tid; i < n_own; i += RES_THREADS) vmin = fmin(vmin, t[i] + dt[i]);
-        for (int off = 16; off > 0; off >>= 1) vmin = fmin(vmin, __shfl_xor_sync(0xffffffffu, vmin, off));
-        if (lane == 0) red[warp] = vmin;
-        __syncthreads();
         if (warp == 0) {
-            vmin = lane < RES_WARPS ? red[lane] : inf;
+            double vmin = inf;
+            for (int i = lane; i < n_own; i += 32) vmin = fmin(vmin, t[i] + dt[i]);
             for (int off = 16; off > 0; off >>= 1) vmin = fmin(vmin, __shfl_xor_sync(0xffffffffu, vmin, off));
             if (lane < C) cluster.map_shared_rank(tmin, lane)[rank] = vmin;
+            if (lane == 0) n_list = 0;   // for the list of the next step (its phase 1 starts after the cluster barrier)
         }
     };
     publish_min();
@@ -159,15 +157,13 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
 
     for (;;) {
         // ---- next block time: every thread of the cluster computes the same minimum
-        double tn = lane < C ? tmin[lane] : inf;
-        for (int off = 16; off > 0; off >>= 1) tn = fmin(tn, __shfl_xor_sync(0xffffffffu, tn, off));
+        double tn = (lane & (RES_MAXC - 1)) < C ? tmin[lane & (RES_MAXC - 1)] : inf;   // both half-warps hold the 16 minima
+        for (int off = RES_MAXC / 2; off > 0; off >>= 1) tn = fmin(tn, __shfl_xor_sync(0xffffffffu, tn, off));
         if (steps_left <= 0 || !(tn <= t_end)) break;
         NB_TICK(0);
 
         // ---- phase 1: predict the owned particles (Eq. 3-7), list the due ones (Table 1 row 1)
-        if (tid == 0) n_list = 0;
-        __syncthreads();
-        for (int i = tid; i < n_own; i += RES_THREADS) {
+        for (int i = tid; i < n_own; i += RES_THREADS) {          // (n_list was reset by publish_min, before the barrier)
             predict_one(i, NL, tn, t, mass, r, v, a, j, s, c, rec);
             if (t[i] + dt[i] == tn) list[atomicAdd(&n_list, 1)] = i;
         }
@@ -176,7 +172,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
         {   // the records of the first RES_PUSH due particles go to every CTA (remote stores, fire and forget)
             const int np = n_list < RES_PUSH ? n_list : RES_PUSH;
             for (int e = tid; e < C * np * REC; e += RES_THREADS) {
-                const int o = e / (np * REC), w = e - o * (np * REC), qq = w / REC, d = w - qq * REC;
+                const int o = e & (C - 1), w = e >> lgC, qq = w / REC, d = w - qq * REC;   // C is a power of two
                 cluster.map_shared_rank(irec, o)[((size_t)rank * RES_PUSH + qq) * REC + d] = rec[(size_t)list[qq] * REC + d];
             }
         }
