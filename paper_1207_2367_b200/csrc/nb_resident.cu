@@ -40,19 +40,21 @@ constexpr int RES_THREADS = 512;    // 16 warps per CTA
 constexpr int RES_WARPS = RES_THREADS / 32;
 constexpr int RES_MAXC = 16;        // largest cluster
 constexpr int RES_NL_MAX = 256;     // owned particles per CTA at most (N <= 2048 on 8 CTAs; 16 CTAs: 128 each)
-constexpr int RES_PUSH = 16;        // each owner pushes the records of its first RES_PUSH due particles to every CTA
+constexpr int RES_PUSH_MIN = 16;    // each owner pushes the records of its first `push` due particles to every CTA: at least
+                                    // this many, and as many more (up to all NL) as the shared memory left over holds
+constexpr size_t RES_SMEM_BUDGET = 227 * 1024 - 2048;   // opt-in shared memory of a CTA on sm_100 less the static part
 
 // Shared-memory plan of one CTA (NL = owned particles, a multiple of 32; doubles unless noted):
 //   state  : t, dt, mass [NL]; r, v, a, jerk, snap, crackle [3][NL]      21 NL
 //   rec    : predicted records [NL][REC]                                   10 NL
 //   f1     : reduced (a, jerk, snap) of the owned active particles [9][NL]  9 NL
 //   part   : partials [C][9][NL] (writer CTA, component, slot), written by every CTA of the cluster   9 C NL
-//   irec   : records of the first RES_PUSH due particles of every CTA [16][RES_PUSH][REC], pushed by their owners
+//   irec   : records of the first `push` due particles of every CTA [16][push][REC], pushed by their owners
 //            (a small active set is then evaluated without a read from remote shared memory)
 //   tmin   : min(t_i + dt_i) of every CTA [16];  list: int32 local indices of the owned due particles [NL];
 //   cnt    : int32 list length of every CTA [16]
 struct ResPlan {
-    int NL, C;
+    int NL, C, push;
     size_t o_t, o_dt, o_m, o_r, o_v, o_a, o_j, o_s, o_c, o_rec, o_f1, o_part, o_irec, o_tmin, o_list, o_cnt, bytes;
 };
 __host__ __device__ inline ResPlan res_plan(const int64_t N, const int C)
@@ -75,7 +77,14 @@ __host__ __device__ inline ResPlan res_plan(const int64_t N, const int C)
     p.o_rec = o; o += (size_t)REC * NL * 8;
     p.o_f1 = o; o += (size_t)9 * NL * 8;
     p.o_part = o; o += (size_t)9 * C * NL * 8;
-    p.o_irec = o; o += (size_t)RES_MAXC * RES_PUSH * REC * 8;
+    {   // irec takes what is left after everything else (the three small arrays below: 16 doubles + NL + 16 ints)
+        const size_t rest = o + (size_t)RES_MAXC * 8 + (size_t)NL * 4 + (size_t)RES_MAXC * 4 + 64;
+        int push = rest < RES_SMEM_BUDGET ? (int)((RES_SMEM_BUDGET - rest) / ((size_t)RES_MAXC * REC * 8)) : 0;
+        if (push > NL) push = NL;
+        if (push < RES_PUSH_MIN) push = RES_PUSH_MIN;
+        p.push = push;
+    }
+    p.o_irec = o; o += (size_t)RES_MAXC * p.push * REC * 8;
     p.o_tmin = o; o += (size_t)RES_MAXC * 8;
     p.o_list = o; o += (size_t)NL * 4;
     p.o_cnt = o; o += (size_t)RES_MAXC * 4;
@@ -97,7 +106,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
     const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
     const int lgC = 31 - __clz(C);                                  // the cluster has 8 or 16 CTAs
     const ResPlan P = res_plan(N, C);
-    const int NL = P.NL;
+    const int NL = P.NL, PUSH = P.push;
     double *t = (double *)(smem + P.o_t), *dt = (double *)(smem + P.o_dt), *mass = (double *)(smem + P.o_m);
     double *r = (double *)(smem + P.o_r), *v = (double *)(smem + P.o_v), *a = (double *)(smem + P.o_a);
     double *j = (double *)(smem + P.o_j), *s = (double *)(smem + P.o_s), *c = (double *)(smem + P.o_c);
@@ -169,11 +178,12 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
         }
         __syncthreads();
         if (tid < C) cluster.map_shared_rank(cnt, tid)[rank] = n_list;
-        {   // the records of the first RES_PUSH due particles go to every CTA (remote stores, fire and forget)
-            const int np = n_list < RES_PUSH ? n_list : RES_PUSH;
-            for (int e = tid; e < C * np * REC; e += RES_THREADS) {
-                const int o = e & (C - 1), w = e >> lgC, qq = w / REC, d = w - qq * REC;   // C is a power of two
-                cluster.map_shared_rank(irec, o)[((size_t)rank * RES_PUSH + qq) * REC + d] = rec[(size_t)list[qq] * REC + d];
+        {   // the records of the first PUSH due particles go to every CTA (remote stores, fire and forget)
+            const int np = n_list < PUSH ? n_list : PUSH;
+            for (int e = tid; e < C * np * (REC / 2); e += RES_THREADS) {   // 16-byte stores; C is a power of two
+                const int o = e & (C - 1), w = e >> lgC, qq = w / (REC / 2), d = w - qq * (REC / 2);
+                reinterpret_cast<double2 *>(cluster.map_shared_rank(irec, o) + ((size_t)rank * PUSH + qq) * REC)[d] =
+                    reinterpret_cast<const double2 *>(rec + (size_t)list[qq] * REC)[d];
             }
         }
         NB_TICK(1);
@@ -218,7 +228,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1)
             }
             const int qloc = kk - bo;                           // slot in the owner's list
             const double *ri;
-            if (qloc < RES_PUSH) ri = irec + ((size_t)o * RES_PUSH + qloc) * REC;     // pushed by its owner in phase 1
+            if (qloc < PUSH) ri = irec + ((size_t)o * PUSH + qloc) * REC;             // pushed by its owner in phase 1
             else ri = cluster.map_shared_rank(rec, o) + (size_t)cluster.map_shared_rank(list, o)[qloc] * REC;
             double rl[REC];                                     // the i-record in five 16-byte loads (local or remote)
 #pragma unroll
